@@ -1,0 +1,153 @@
+"""ORACLE -- test infrastructure, not product code.
+
+ctypes wrapper around oracle/ts_oracle.c (the plain single-threaded CPU restatement of the
+paper's per-vehicle traffic microsimulation).  Only tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import this
+package; nothing under paper_1807_01148_b200/ does, and this package imports nothing from it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+_PARAM_FIELDS = [
+    ("dt", C.c_float), ("a", C.c_float), ("b", C.c_float), ("T", C.c_float), ("s0", C.c_float),
+    ("veh_len", C.c_float), ("b_safe", C.c_float), ("politeness", C.c_float),
+    ("lc_threshold", C.c_float), ("mand_dist_default", C.c_float),
+    ("lookahead_cells", C.c_uint32), ("lookback_cells", C.c_uint32), ("lc_period", C.c_uint32),
+    ("entry_zone_cells", C.c_uint32), ("insert_clear_cells", C.c_uint32),
+    ("sample_period_steps", C.c_uint32),
+]
+
+
+class OrcParams(C.Structure):
+    _fields_ = _PARAM_FIELDS
+
+
+_COUNTER_NAMES = ["updates", "own_cells", "next_cells", "lc_evals", "lc_cells", "lc_accepts",
+                  "lc_mandatory", "crossings", "cross_lost", "held_red", "cap_bound",
+                  "departures", "arrivals", "peak_active"]
+
+
+class OrcCounters(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in _COUNTER_NAMES]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build())
+        L.orc_create.restype = C.c_void_p
+        L.orc_create.argtypes = [C.c_uint32, C.c_uint32] + [C.c_void_p] * 9 + [C.c_uint32] + [C.c_void_p] * 5 + [C.POINTER(OrcParams)]
+        L.orc_step.restype = C.c_int
+        L.orc_step.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_int, C.c_uint64]
+        L.orc_read_state.restype = None
+        L.orc_read_state.argtypes = [C.c_void_p] * 14
+        L.orc_read_edge_stats.restype = None
+        L.orc_read_edge_stats.argtypes = [C.c_void_p] * 7 + [C.c_int]
+        L.orc_get_counters.restype = None
+        L.orc_get_counters.argtypes = [C.c_void_p, C.POINTER(OrcCounters)]
+        L.orc_destroy.restype = None
+        L.orc_destroy.argtypes = [C.c_void_p]
+        L.orc_last_error.restype = C.c_char_p
+        L.orc_idm.restype = C.c_float
+        L.orc_idm.argtypes = [C.POINTER(OrcParams), C.c_float, C.c_float, C.c_int, C.c_float, C.c_float]
+        L.orc_speed_code.restype = C.c_uint8
+        L.orc_speed_code.argtypes = [C.c_float]
+        L.orc_speed_decode.restype = C.c_float
+        L.orc_speed_decode.argtypes = [C.c_uint8]
+        L.orc_signal_green.restype = C.c_int
+        L.orc_signal_green.argtypes = [C.c_uint32] * 5 + [C.c_uint64]
+        L.orc_mix64.restype = C.c_uint64
+        L.orc_mix64.argtypes = [C.c_uint64]
+        _lib = L
+    return _lib
+
+
+def make_params(d) -> OrcParams:
+    p = OrcParams()
+    for name, _ in _PARAM_FIELDS:
+        setattr(p, name, d[name])
+    return p
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+class Oracle:
+    """One simulation.  `bundle` is a dict as produced by the workload module."""
+
+    def __init__(self, bundle):
+        L = lib()
+        b = bundle
+        self.V, self.E = int(b["n_vehicles"]), int(b["n_edges"])
+        self._p = make_params(b["params"])
+        self._keep = [np.ascontiguousarray(b[k]) for k in (
+            "edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim", "node_ctrl",
+            "sig_green_steps", "sig_allred_steps", "sig_offset_steps", "route_off", "route_edges",
+            "depart_time_s", "v0_mult", "mand_dist_m")]
+        k = self._keep
+        self._h = L.orc_create(int(b["n_nodes"]), self.E, *[_ptr(a) for a in k[:9]], self.V,
+                               *[_ptr(a) for a in k[9:]], C.byref(self._p))
+        if not self._h:
+            raise OracleError(L.orc_last_error().decode())
+
+    def step(self, n, digests=False, check=0, order_seed=0):
+        d = np.zeros(n, np.uint64) if digests else None
+        if lib().orc_step(self._h, int(n), _ptr(d), int(check), int(order_seed)) != 0:
+            raise OracleError(lib().orc_last_error().decode())
+        return d
+
+    def read_state(self):
+        V = self.V
+        out = dict(status=np.zeros(V, np.uint8), edge=np.zeros(V, np.uint32), lane=np.zeros(V, np.uint8),
+                   cell=np.zeros(V, np.uint32), x=np.zeros(V, np.float32), v=np.zeros(V, np.float32),
+                   route_idx=np.zeros(V, np.uint32), insert_step=np.zeros(V, np.uint32),
+                   arrive_step=np.zeros(V, np.uint32))
+        step = C.c_uint64(); npend = C.c_uint32(); nact = C.c_uint32(); narr = C.c_uint32()
+        lib().orc_read_state(self._h, *[_ptr(out[k]) for k in ("status", "edge", "lane", "cell", "x", "v", "route_idx", "insert_step", "arrive_step")],
+                             C.addressof(step), C.addressof(npend), C.addressof(nact), C.addressof(narr))
+        out.update(step=step.value, n_pending=npend.value, n_active=nact.value, n_arrived=narr.value)
+        return out
+
+    def read_edge_stats(self, reset=False):
+        E = self.E
+        out = dict(entered=np.zeros(E, np.uint32), exited=np.zeros(E, np.uint32),
+                   exit_steps_sum=np.zeros(E, np.uint64), sample_count_sum=np.zeros(E, np.uint32),
+                   sample_speedcode_sum=np.zeros(E, np.uint64))
+        ns = C.c_uint32()
+        lib().orc_read_edge_stats(self._h, *[_ptr(out[k]) for k in ("entered", "exited", "exit_steps_sum", "sample_count_sum", "sample_speedcode_sum")],
+                                  C.addressof(ns), int(bool(reset)))
+        out["n_samples"] = ns.value
+        return out
+
+    def counters(self):
+        c = OrcCounters()
+        lib().orc_get_counters(self._h, C.byref(c))
+        return {n: getattr(c, n) for n in _COUNTER_NAMES}
+
+    def close(self):
+        if self._h:
+            lib().orc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def idm(params, v, v0, has_leader, s, dv):
+    return float(lib().orc_idm(C.byref(make_params(params)), v, v0, int(has_leader), s, dv))

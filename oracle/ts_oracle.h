@@ -1,0 +1,120 @@
+/*
+ * ts_oracle.h -- ORACLE (test infrastructure, not product code).
+ *
+ * A plain, slow, single-threaded CPU restatement of the per-vehicle traffic
+ * microsimulation of arxiv 1807.01148 (sections 6.3.2-6.3.3), following
+ * SURVEY.md section 8(c) step by step (readings R1-R22 are listed in DESIGN.md).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+ * may load this library.  It shares no code, header, table or helper with the CUDA path
+ * under paper_1807_01148_b200/csrc/ and never includes include/trafficsim.h.
+ *
+ * Where the paper says the GPU method "represent[s] a road as a set of contiguous bytes"
+ * and finds the leader by "check[ing] the following bytes", the oracle
+ * deliberately does NOT build a byte map: it keeps an ordered list of vehicles per lane
+ * ("a list of vehicles per lane", the structure the paper says it replaced) and applies
+ * the same perception rule (cell index + quantised speed code).  orc_check() re-derives
+ * every neighbour by an O(V^2) search over raw (edge, lane, x) as a second, independent
+ * route to the same answer.
+ *
+ * Parity pins (tests/test_oracle_pins.py): P1 lone-vehicle closed form, P2 platoon
+ * equilibrium gap, P3 standing queue, I1-I8 invariants, P4 brute force, P5 degenerate cases.
+ * PARITY UNPINNED against the outside world (pinned oracle<->GPU only): the MOBIL
+ * incentive values, hold-at-line behaviour and departure ordering (SURVEY.md:425-426).
+ */
+#ifndef TS_ORACLE_H
+#define TS_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Model parameters (PAPER.md:390 dt; :394-397 IDM a,b,T,s0; :399-400 lane change). */
+typedef struct orc_params {
+    float dt;            /* time step, s (0.5) */
+    float a;             /* IDM acceleration ability, m/s^2 */
+    float b;             /* IDM comfortable braking, m/s^2 */
+    float T;             /* IDM desired time headway, s */
+    float s0;            /* IDM minimum following distance, m */
+    float veh_len;       /* vehicle length, m */
+    float b_safe;        /* gap acceptance: max braking imposed on the new follower */
+    float politeness;    /* MOBIL politeness p */
+    float lc_threshold;  /* MOBIL incentive threshold, m/s^2 */
+    float mand_dist_default; /* used where mand_dist_m == NULL */
+    uint32_t lookahead_cells;     /* H  */
+    uint32_t lookback_cells;      /* Hb */
+    uint32_t lc_period;           /* 0 = lane changes disabled */
+    uint32_t entry_zone_cells;
+    uint32_t insert_clear_cells;
+    uint32_t sample_period_steps; /* 0 = no sampling */
+} orc_params;
+
+/* Work counters: what a byte-scan method would have to touch. */
+typedef struct orc_counters {
+    uint64_t updates;          /* ACTIVE vehicle advanced one step */
+    uint64_t own_cells;        /* cells between a vehicle and its leader / scan limit, own edge */
+    uint64_t next_cells;       /* same, on the next route edge */
+    uint64_t lc_evals;         /* lane-change evaluations */
+    uint64_t lc_cells;         /* target-lane cells (ahead + behind) examined */
+    uint64_t lc_accepts;
+    uint64_t lc_mandatory;
+    uint64_t crossings;        /* winning edge transitions */
+    uint64_t cross_lost;       /* CROSS intents that lost a claim */
+    uint64_t held_red;         /* held at a red stop line */
+    uint64_t cap_bound;        /* advance limited by the no-overlap cap */
+    uint64_t departures;
+    uint64_t arrivals;
+    uint64_t peak_active;
+} orc_counters;
+
+typedef struct orc_sim orc_sim;
+
+/* All pointers are host arrays owned by the caller and copied.  v0_mult / mand_dist_m may
+ * be NULL.  Returns NULL on invalid input (message in orc_last_error()). */
+orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
+                    const uint32_t *edge_from, const uint32_t *edge_to,
+                    const uint32_t *edge_len_m, const uint8_t *edge_lanes,
+                    const float *edge_vlim, const uint8_t *node_ctrl,
+                    const uint32_t *sig_green_steps, const uint32_t *sig_allred_steps,
+                    const uint32_t *sig_offset_steps,
+                    uint32_t n_vehicles, const uint64_t *route_off,
+                    const uint32_t *route_edges, const float *depart_time_s,
+                    const float *v0_mult, const float *mand_dist_m,
+                    const orc_params *params);
+
+/* Advance n steps.  digests (nullable) receives one 64-bit digest per step (state k+1).
+ * check: 0 none, 1 invariants I1-I7 every step, 2 additionally the O(V^2) brute-force
+ * neighbour search (P4).  order_seed != 0 permutes the vehicle iteration order (I8).
+ * Returns 0, or -1 on an invariant violation (message in orc_last_error()). */
+int orc_step(orc_sim *s, uint32_t n, uint64_t *digests, int check, uint64_t order_seed);
+
+/* Length-V arrays in vehicle-id order; any pointer may be NULL. */
+void orc_read_state(const orc_sim *s, uint8_t *status, uint32_t *edge, uint8_t *lane,
+                    uint32_t *cell, float *x, float *v, uint32_t *route_idx,
+                    uint32_t *insert_step, uint32_t *arrive_step,
+                    uint64_t *step, uint32_t *n_pending, uint32_t *n_active,
+                    uint32_t *n_arrived);
+
+/* Length-E arrays; any pointer may be NULL. */
+void orc_read_edge_stats(orc_sim *s, uint32_t *entered, uint32_t *exited,
+                         uint64_t *exit_steps_sum, uint32_t *sample_count_sum,
+                         uint64_t *sample_speedcode_sum, uint32_t *n_samples, int reset);
+
+void orc_get_counters(const orc_sim *s, orc_counters *out);
+void orc_destroy(orc_sim *s);
+const char *orc_last_error(void);
+
+/* Scalar building blocks exported so the pins can probe them directly. */
+float orc_idm(const orc_params *p, float v, float v0, int has_leader, float s, float dv);
+uint8_t orc_speed_code(float v);
+float orc_speed_decode(uint8_t code);
+int orc_signal_green(uint32_t green, uint32_t allred, uint32_t offset, uint32_t n_in,
+                     uint32_t in_rank, uint64_t k);
+uint64_t orc_mix64(uint64_t z);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
