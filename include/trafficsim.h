@@ -1,0 +1,179 @@
+/*
+ * trafficsim.h -- C ABI of the B200-native traffic microsimulation (libts.so).
+ *
+ * What it computes: the time-stepped, per-vehicle traffic simulation of arxiv 1807.01148,
+ * section 6.3.2 "Per-vehicle and traffic control simulation" (Intelligent
+ * Driver Model car following Eq. 7, mandatory/discretionary lane changes, gap acceptance,
+ * stop and traffic-light control) on the "traffic atlas" of section 6.3.3 (PAPER.md:404-406:
+ * "we represent a road as a set of contiguous bytes in memory, in order to find the leading
+ * car of a given vehicle, we check the following bytes"), along per-vehicle paths
+ * (PAPER.md:370, :382-384), with the outputs of section 6.4.
+ * The exact rule set (one synchronous step k -> k+1, readings R1-R22 where the paper is
+ * silent) is written out in DESIGN.md sections 2-3.
+ *
+ * Conventions
+ *  - No global state, no exceptions, no allocation on the device by the library: the caller
+ *    owns ONE device workspace (size from ts_query_workspace) and a CUDA stream.
+ *  - Every pointer inside ts_network / ts_routes / ts_departures is a HOST pointer owned by
+ *    the caller; ts_create copies what it needs and keeps no pointer afterwards.
+ *  - Output pointers (ts_state_out, ts_edge_stats_out, digests) are HOST pointers unless
+ *    ts_device.out_on_device != 0, in which case they are DEVICE pointers.
+ *  - All calls on one ts_sim must come from one thread at a time.  Work is enqueued on
+ *    ts_device.cuda_stream; ts_step is asynchronous, the ts_read_* calls synchronise.
+ *  - Return value: TS_OK (0) or a negative ts_status; ts_last_error() gives the message.
+ *  - fp32 state is reproducible bit for bit: kernels are built with -fmad=false and IEEE
+ *    division; arbitration is by lowest vehicle id with integer atomics only.
+ *  - There is no CPU fallback: without a CUDA device every call but ts_query_workspace,
+ *    ts_last_error and ts_version fails with TS_ECUDA.
+ */
+#ifndef TRAFFICSIM_H
+#define TRAFFICSIM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum ts_status {
+    TS_OK = 0,
+    TS_EINVAL = -1,     /* bad sizes, non-contiguous route, lanes not in 1..8, edge shorter than
+                           16 or longer than 65535 cells, entry zone too short for the fastest
+                           vehicle, lookahead not a multiple of 16, ... */
+    TS_ENOMEM = -2,     /* workspace too small */
+    TS_ECUDA = -3,      /* CUDA runtime error (or no device) */
+    TS_EINVARIANT = -4  /* device-side sticky flag: two vehicles scattered to one cell */
+} ts_status;
+
+/* Node control types ("stop and traffic light signals"). */
+enum { TS_CTRL_FREE = 0, TS_CTRL_PRIORITY = 1, TS_CTRL_SIGNAL = 2 };
+/* Vehicle status. */
+enum { TS_PENDING = 0, TS_ACTIVE = 1, TS_ARRIVED = 2 };
+
+/* The road network (nodes, directional edges, per-edge speed and lanes). */
+typedef struct ts_network {
+    uint32_t n_nodes, n_edges;
+    const uint32_t *edge_from;        /* [E] tail node */
+    const uint32_t *edge_to;          /* [E] head node */
+    const uint32_t *edge_len_m;       /* [E] length in cells = metres, 16..65535 */
+    const uint8_t *edge_lanes;        /* [E] 1..8, lane 0 = kerb side */
+    const float *edge_vlim;           /* [E] speed limit m/s, > 0 */
+    const uint8_t *node_ctrl;         /* [N] TS_CTRL_* of the node at the head of an edge */
+    const uint32_t *sig_green_steps;  /* [N] read where ctrl == SIGNAL; >= 1; green+allred <= 65535 */
+    const uint32_t *sig_allred_steps; /* [N] */
+    const uint32_t *sig_offset_steps; /* [N] < 2^31 */
+} ts_network;
+
+/* Per-vehicle paths.  Vehicle id = index.  Each route has >= 1 edge and
+ * head(route[j]) == tail(route[j+1]). */
+typedef struct ts_routes {
+    uint32_t n_vehicles;
+    const uint64_t *route_off;        /* [V+1] */
+    const uint32_t *route_edges;      /* [route_off[V]] */
+} ts_routes;
+
+/* Departure times and per-vehicle procedural variables. */
+typedef struct ts_departures {
+    const float *depart_time_s;       /* [V] >= 0; departs at step ceil(t/dt) or later */
+    const float *v0_mult;             /* [V] desired speed = v0_mult * edge limit; NULL => 1 */
+    const float *mand_dist_m;         /* [V] distance to the exit at which a wrong-lane vehicle
+                                         turns mandatory; NULL => default */
+} ts_departures;
+
+/* Model parameters.  Defaults in DESIGN.md section 3 (BASELINE.json configs 1-2). */
+typedef struct ts_params {
+    float dt;                 /* s, PAPER.md:390 (0.5) */
+    float a, b, T, s0;        /* IDM, Eq. 7 */
+    float veh_len;            /* m, >= 2 */
+    float b_safe;             /* gap acceptance: max braking imposed on the lag vehicle */
+    float politeness;         /* MOBIL p */
+    float lc_threshold;       /* MOBIL incentive threshold m/s^2 */
+    float mand_dist_default;  /* m */
+    uint32_t lookahead_cells; /* H: multiple of 16, 16..4096 */
+    uint32_t lookback_cells;  /* Hb */
+    uint32_t lc_period;       /* lane change evaluated when ((k>>1)+id) % lc_period == 0; 0 = never */
+    uint32_t entry_zone_cells;   /* no lane change in the first cells of an edge */
+    uint32_t insert_clear_cells; /* 1..16: cells of lane 0 that must be empty to insert */
+    uint32_t sample_period_steps;/* PAPER.md:437 (120 = one minute); 0 = never */
+} ts_params;
+
+/* Device resources lent by the caller for the lifetime of the ts_sim. */
+typedef struct ts_device {
+    void *workspace;          /* DEVICE pointer, 256-byte aligned */
+    size_t bytes;             /* >= ts_query_workspace */
+    void *cuda_stream;        /* cudaStream_t (NULL = legacy default stream) */
+    int out_on_device;        /* non-zero: ts_read_* / digest outputs are device pointers */
+} ts_device;
+
+/* Length-V arrays in vehicle-id order (any pointer may be NULL), plus scalars. */
+typedef struct ts_state_out {
+    uint8_t *status;          /* TS_PENDING / TS_ACTIVE / TS_ARRIVED */
+    uint32_t *edge;           /* current edge (first route edge while pending, last when arrived) */
+    uint8_t *lane;
+    uint32_t *cell;           /* floor(x) */
+    float *x;                 /* m from the edge start (front bumper); == edge length once arrived */
+    float *v;                 /* m/s */
+    uint32_t *route_idx;      /* index into the vehicle's route */
+    uint32_t *insert_step;    /* step at which it became ACTIVE (0 while pending) */
+    uint32_t *arrive_step;    /* step at which it ARRIVED (0 before) */
+    /* scalars, always written (host memory, whatever out_on_device says) */
+    uint64_t step;
+    uint32_t n_pending, n_active, n_arrived;
+    uint64_t vehicle_updates; /* sum over steps of ACTIVE vehicles advanced (the bench metric) */
+} ts_state_out;
+
+/* Length-E integer accumulators (PAPER.md:437 samples; PAPER.md:446 utilisation is derived
+ * on the host: sample_count_sum / n_samples / (len * lanes / (veh_len + s0))). */
+typedef struct ts_edge_stats_out {
+    uint32_t *entered;               /* vehicles that entered the edge (departures included) */
+    uint32_t *exited;                /* vehicles that left it (arrivals included) */
+    uint64_t *exit_steps_sum;        /* sum over exits of steps spent on the edge */
+    uint32_t *sample_count_sum;      /* sum over samples of vehicles on the edge */
+    uint64_t *sample_speedcode_sum;  /* sum over samples and vehicles of round(4 v) (0.25 m/s units) */
+    uint32_t n_samples;              /* always host */
+} ts_edge_stats_out;
+
+typedef struct ts_sim ts_sim;
+
+/* Device bytes ts_create needs for these inputs.  Pure host arithmetic; validates sizes only. */
+int ts_query_workspace(const ts_network *net, const ts_routes *routes,
+                       const ts_departures *dep, const ts_params *params, size_t *bytes);
+
+/* Validate, lay out the workspace, copy the inputs (H2D on dev->cuda_stream) and set the
+ * state of step 0: every vehicle PENDING, atlas empty.  *out is NULL on failure. */
+int ts_create(const ts_network *net, const ts_routes *routes, const ts_departures *dep,
+              const ts_params *params, const ts_device *dev, ts_sim **out);
+
+/* Enqueue n steps (one step = DESIGN.md section 2, steps 1-5).  Asynchronous. */
+int ts_step(ts_sim *sim, uint32_t n);
+
+/* Same, and writes one 64-bit state digest per step to digests[0..n) (DESIGN.md section 2.6:
+ * order-independent sum of SplitMix64-mixed (id, edge, lane, bits(x), bits(v)) over ACTIVE
+ * vehicles plus a mix of the counters).  Synchronises when digests is a host pointer. */
+int ts_step_digest(ts_sim *sim, uint32_t n, uint64_t *digests);
+
+/* Back to step 0 without re-uploading the inputs. */
+int ts_reset(ts_sim *sim);
+
+/* Snapshot in vehicle-id order.  Synchronises; reports the sticky TS_EINVARIANT if raised. */
+int ts_read_state(ts_sim *sim, ts_state_out *out);
+int ts_read_edge_stats(ts_sim *sim, ts_edge_stats_out *out, int reset);
+
+/* Tuning knobs that never change results.  "mode": 1 (default) = ts_step(n) is ONE persistent
+ * cooperative kernel looping over the n steps with grid-wide barriers; 0 = two launches per
+ * step.  "blocks_per_sm": resident CTAs per SM of the step kernels (1..occupancy limit). */
+int ts_set_option(ts_sim *sim, const char *key, long long value);
+
+/* Frees host bookkeeping only; the workspace stays the caller's. */
+void ts_destroy(ts_sim *sim);
+
+/* Thread-local message of the last non-zero return. */
+const char *ts_last_error(void);
+/* "major.minor (build flags)" */
+const char *ts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRAFFICSIM_H */

@@ -1,0 +1,219 @@
+"""Thin ctypes binding of libts.so (include/trafficsim.h): argument marshalling only.
+
+PyTorch is used for what the header asks the caller to provide: one device workspace tensor
+and a CUDA stream.  Every step of the simulation runs in the library's kernels; there is no
+Python or CPU fallback, and loading fails loudly if the library has not been built."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libts.so")
+
+TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
+
+EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
+           "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_destroy", "ts_last_error",
+           "ts_version"]
+
+_u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
+                             C.POINTER(C.c_uint64))
+
+
+class TsNetwork(C.Structure):
+    _fields_ = [("n_nodes", C.c_uint32), ("n_edges", C.c_uint32), ("edge_from", C.c_void_p),
+                ("edge_to", C.c_void_p), ("edge_len_m", C.c_void_p), ("edge_lanes", C.c_void_p),
+                ("edge_vlim", C.c_void_p), ("node_ctrl", C.c_void_p), ("sig_green_steps", C.c_void_p),
+                ("sig_allred_steps", C.c_void_p), ("sig_offset_steps", C.c_void_p)]
+
+
+class TsRoutes(C.Structure):
+    _fields_ = [("n_vehicles", C.c_uint32), ("route_off", C.c_void_p), ("route_edges", C.c_void_p)]
+
+
+class TsDepartures(C.Structure):
+    _fields_ = [("depart_time_s", C.c_void_p), ("v0_mult", C.c_void_p), ("mand_dist_m", C.c_void_p)]
+
+
+class TsParams(C.Structure):
+    _fields_ = [(n, C.c_float) for n in ("dt", "a", "b", "T", "s0", "veh_len", "b_safe", "politeness",
+                                         "lc_threshold", "mand_dist_default")] + \
+               [(n, C.c_uint32) for n in ("lookahead_cells", "lookback_cells", "lc_period",
+                                          "entry_zone_cells", "insert_clear_cells", "sample_period_steps")]
+
+
+class TsDevice(C.Structure):
+    _fields_ = [("workspace", C.c_void_p), ("bytes", C.c_size_t), ("cuda_stream", C.c_void_p),
+                ("out_on_device", C.c_int)]
+
+
+class TsStateOut(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("status", "edge", "lane", "cell", "x", "v", "route_idx",
+                                          "insert_step", "arrive_step")] + \
+               [("step", C.c_uint64), ("n_pending", C.c_uint32), ("n_active", C.c_uint32),
+                ("n_arrived", C.c_uint32), ("vehicle_updates", C.c_uint64)]
+
+
+class TsEdgeStatsOut(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("entered", "exited", "exit_steps_sum", "sample_count_sum",
+                                          "sample_speedcode_sum")] + [("n_samples", C.c_uint32)]
+
+
+class TsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"ts error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """dlopen libts.so.  No fallback: a missing library is an error."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is not built: run `python -m paper_1807_01148_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.ts_query_workspace.argtypes = [C.c_void_p] * 4 + [C.POINTER(C.c_size_t)]
+        L.ts_create.argtypes = [C.c_void_p] * 5 + [C.POINTER(C.c_void_p)]
+        L.ts_step.argtypes = [C.c_void_p, C.c_uint32]
+        L.ts_step_digest.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p]
+        L.ts_reset.argtypes = [C.c_void_p]
+        L.ts_read_state.argtypes = [C.c_void_p, C.c_void_p]
+        L.ts_read_edge_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.ts_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
+        L.ts_destroy.argtypes = [C.c_void_p]
+        L.ts_destroy.restype = None
+        L.ts_last_error.restype = C.c_char_p
+        L.ts_version.restype = C.c_char_p
+        for n in EXPORTS[:8]:
+            getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise TsError(rc, load().ts_last_error().decode())
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data
+
+
+def marshal(bundle):
+    """bundle dict -> (net, routes, dep, params, keepalive)."""
+    b = bundle
+    keep = {k: np.ascontiguousarray(b[k]) for k in (
+        "edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim", "node_ctrl",
+        "sig_green_steps", "sig_allred_steps", "sig_offset_steps", "route_off", "route_edges",
+        "depart_time_s")}
+    for k in ("v0_mult", "mand_dist_m"):
+        keep[k] = None if b.get(k) is None else np.ascontiguousarray(b[k])
+    net = TsNetwork(int(b["n_nodes"]), int(b["n_edges"]), *[_p(keep[k]) for k in (
+        "edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim", "node_ctrl",
+        "sig_green_steps", "sig_allred_steps", "sig_offset_steps")])
+    routes = TsRoutes(int(b["n_vehicles"]), _p(keep["route_off"]), _p(keep["route_edges"]))
+    dep = TsDepartures(_p(keep["depart_time_s"]), _p(keep["v0_mult"]), _p(keep["mand_dist_m"]))
+    prm = TsParams(**{n: b["params"][n] for n, _ in TsParams._fields_})
+    return net, routes, dep, prm, keep
+
+
+def query_workspace(bundle) -> int:
+    net, routes, dep, prm, _keep = marshal(bundle)
+    n = C.c_size_t()
+    _check(load().ts_query_workspace(C.byref(net), C.byref(routes), C.byref(dep), C.byref(prm), C.byref(n)))
+    return n.value
+
+
+class Sim:
+    """ts_create / ts_step / ts_read_state / ts_read_edge_stats on one GPU."""
+
+    def __init__(self, bundle, device="cuda:0", stream=None, mode=None):
+        import torch
+        L = load()
+        self.V, self.E = int(bundle["n_vehicles"]), int(bundle["n_edges"])
+        net, routes, dep, prm, keep = marshal(bundle)
+        self.workspace_bytes = query_workspace(bundle)
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self._ws.data_ptr() + 255) & ~255
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        dev = TsDevice(base, self.workspace_bytes, self._stream.cuda_stream, 0)
+        h = C.c_void_p()
+        _check(L.ts_create(C.byref(net), C.byref(routes), C.byref(dep), C.byref(prm), C.byref(dev), C.byref(h)))
+        self._h = h
+        if mode is not None:
+            self.set_option("mode", mode)
+
+    def set_option(self, key, value):
+        _check(load().ts_set_option(self._h, key.encode(), int(value)))
+
+    def step(self, n):
+        _check(load().ts_step(self._h, int(n)))
+
+    def step_digest(self, n):
+        d = np.zeros(int(n), np.uint64)
+        _check(load().ts_step_digest(self._h, int(n), d.ctypes.data))
+        return d
+
+    def reset(self):
+        _check(load().ts_reset(self._h))
+
+    def read_state(self):
+        V = self.V
+        out = dict(status=np.zeros(V, np.uint8), edge=np.zeros(V, np.uint32), lane=np.zeros(V, np.uint8),
+                   cell=np.zeros(V, np.uint32), x=np.zeros(V, np.float32), v=np.zeros(V, np.float32),
+                   route_idx=np.zeros(V, np.uint32), insert_step=np.zeros(V, np.uint32),
+                   arrive_step=np.zeros(V, np.uint32))
+        o = TsStateOut(*[_p(out[k]) for k in ("status", "edge", "lane", "cell", "x", "v", "route_idx",
+                                               "insert_step", "arrive_step")])
+        _check(load().ts_read_state(self._h, C.byref(o)))
+        out.update(step=o.step, n_pending=o.n_pending, n_active=o.n_active, n_arrived=o.n_arrived,
+                   vehicle_updates=o.vehicle_updates)
+        return out
+
+    def read_counts(self):
+        """Scalars only (no per-vehicle arrays are copied)."""
+        o = TsStateOut()
+        _check(load().ts_read_state(self._h, C.byref(o)))
+        return dict(step=o.step, n_pending=o.n_pending, n_active=o.n_active, n_arrived=o.n_arrived,
+                    vehicle_updates=o.vehicle_updates)
+
+    def read_edge_stats(self, reset=False):
+        E = self.E
+        out = dict(entered=np.zeros(E, np.uint32), exited=np.zeros(E, np.uint32),
+                   exit_steps_sum=np.zeros(E, np.uint64), sample_count_sum=np.zeros(E, np.uint32),
+                   sample_speedcode_sum=np.zeros(E, np.uint64))
+        o = TsEdgeStatsOut(*[_p(out[k]) for k in ("entered", "exited", "exit_steps_sum",
+                                                   "sample_count_sum", "sample_speedcode_sum")])
+        _check(load().ts_read_edge_stats(self._h, C.byref(o), int(bool(reset))))
+        out["n_samples"] = o.n_samples
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load().ts_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def utilisation(edge_stats, bundle):
+    """vehicles on the edge at the sampling time divided by the number that fit:
+    length x lanes / (vehicle length + lead gap), averaged over the samples taken."""
+    p = bundle["params"]
+    cap = bundle["edge_len_m"].astype(np.float64) * bundle["edge_lanes"] / (p["veh_len"] + p["s0"])
+    n = max(1, int(edge_stats["n_samples"]))
+    return edge_stats["sample_count_sum"] / n / cap

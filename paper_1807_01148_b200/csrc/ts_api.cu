@@ -1,0 +1,563 @@
+// ts_api.cu -- C ABI (include/trafficsim.h) and kernels of libts.so.  Product code, sm_100a.
+//
+// Host side: validation, workspace layout, upload.  Device side: thin __global__ wrappers
+// around the phases in ts_phases.cuh, either two launches per step (mode 0) or ONE persistent
+// cooperative kernel per ts_step(n) call that loops over the n steps with grid-wide barriers
+// (mode 1, default): the step is bound by the two grid-wide dependencies, not by bandwidth,
+// so no host launch may sit inside the loop.
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "../../include/trafficsim.h"
+#include "ts_phases.cuh"
+
+namespace cg = cooperative_groups;
+using namespace ts;
+
+// ------------------------------------------------------------------ errors
+
+static thread_local char g_err[512] = "";
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define CUDA_TRY(call)                                                                    \
+    do {                                                                                  \
+        cudaError_t e_ = (call);                                                          \
+        if (e_ != cudaSuccess)                                                            \
+            return fail(TS_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+extern "C" const char* ts_last_error(void) { return g_err; }
+extern "C" const char* ts_version(void) {
+    return "0.1 (sm_100a, -fmad=false, IEEE div/sqrt, single-buffer atlas, persistent step kernel)";
+}
+
+// ------------------------------------------------------------------ layout
+
+struct Layout {
+    size_t total = 0;
+    uint32_t V = 0, E = 0, N = 0, Q = 0, cap = 0;
+    uint64_t R = 0, n_lanes = 0, atlas_bytes = 0;
+    size_t edges, route_edges, route_begin, route_end, v0_mult, mand_dist, queue_edge, queue_off,
+        queue_veh, queue_dep, atlas, queue_head, queue_cand, lane_claim, node_claim, dyn, slots,
+        o_status, o_lane, o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered,
+        st_exited, st_exit_steps, st_samp_cnt, st_samp_code, digest;
+    static constexpr uint32_t kSlotArrays = 13;
+    static constexpr uint32_t kDigestChunk = 8192;
+    size_t take(size_t bytes) {
+        size_t off = total;
+        total += (bytes + 255) & ~(size_t)255;
+        return off;
+    }
+    void plan() {
+        edges = take((size_t)E * sizeof(EdgeRec));
+        route_edges = take(R * 4);
+        route_begin = take((size_t)V * 4); route_end = take((size_t)V * 4);
+        v0_mult = take((size_t)V * 4); mand_dist = take((size_t)V * 4);
+        queue_edge = take((size_t)Q * 4); queue_off = take(((size_t)Q + 1) * 4);
+        queue_veh = take((size_t)V * 4); queue_dep = take((size_t)V * 4);
+        atlas = take(atlas_bytes);
+        queue_head = take((size_t)Q * 4); queue_cand = take((size_t)Q * 4);
+        lane_claim = take(n_lanes * 8); node_claim = take((size_t)N * 8);
+        dyn = take(sizeof(Dyn));
+        slots = take((size_t)cap * 4 * kSlotArrays);
+        o_status = take(V); o_lane = take(V);
+        o_edge = take((size_t)V * 4); o_x = take((size_t)V * 4); o_v = take((size_t)V * 4);
+        o_rpos = take((size_t)V * 4); o_insert = take((size_t)V * 4); o_arrive = take((size_t)V * 4);
+        o_cell = take((size_t)V * 4); o_ridx = take((size_t)V * 4);
+        st_entered = take((size_t)E * 4); st_exited = take((size_t)E * 4);
+        st_exit_steps = take((size_t)E * 8); st_samp_cnt = take((size_t)E * 4);
+        st_samp_code = take((size_t)E * 8);
+        digest = take((size_t)kDigestChunk * 8);
+    }
+};
+
+// Sizes only (what ts_query_workspace may look at).
+static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
+    if (!net || !rt) return fail(TS_EINVAL, "null argument");
+    if (net->n_edges == 0 || net->n_nodes == 0) return fail(TS_EINVAL, "empty network");
+    if (rt->n_vehicles >= 0xFFFFFFFEu) return fail(TS_EINVAL, "too many vehicles");
+    L.V = rt->n_vehicles; L.E = net->n_edges; L.N = net->n_nodes;
+    L.R = L.V ? rt->route_off[L.V] : 0;
+    if (L.R >= 0xFFFFFFFEull) return fail(TS_EINVAL, "route table too long (%llu entries)", (unsigned long long)L.R);
+    uint64_t rows16 = 0, lanes = 0;
+    for (uint32_t e = 0; e < L.E; e++) {
+        uint32_t ln = net->edge_lanes[e], len = net->edge_len_m[e];
+        if (ln < 1 || ln > 8) return fail(TS_EINVAL, "edge %u: lanes %u not in 1..8", e, ln);
+        if (len < 16 || len > 65535) return fail(TS_EINVAL, "edge %u: length %u not in 16..65535", e, len);
+        rows16 += (uint64_t)ln * ((len + 15) >> 4);
+        lanes += ln;
+    }
+    if (rows16 >= 0xFFFFFFFFull) return fail(TS_EINVAL, "atlas larger than 64 GiB");
+    L.atlas_bytes = rows16 * 16; L.n_lanes = lanes;
+    std::vector<uint8_t> is_origin(L.E, 0);
+    uint32_t q = 0;
+    for (uint32_t i = 0; i < L.V; i++) {
+        if (rt->route_off[i + 1] <= rt->route_off[i]) return fail(TS_EINVAL, "vehicle %u: empty route", i);
+        uint32_t e = rt->route_edges[rt->route_off[i]];
+        if (e >= L.E) return fail(TS_EINVAL, "vehicle %u: route edge %u out of range", i, e);
+        if (!is_origin[e]) { is_origin[e] = 1; q++; }
+    }
+    L.Q = q; L.cap = L.V;   // every vehicle takes exactly one slot in its life
+    L.plan();
+    return TS_OK;
+}
+
+extern "C" int ts_query_workspace(const ts_network* net, const ts_routes* routes, const ts_departures* dep,
+                                  const ts_params* params, size_t* bytes) {
+    (void)dep; (void)params;
+    if (!bytes) return fail(TS_EINVAL, "bytes is null");
+    Layout L;
+    int rc = plan_sizes(net, routes, L);
+    if (rc) return rc;
+    *bytes = L.total;
+    return TS_OK;
+}
+
+// ------------------------------------------------------------------ the simulation object
+
+struct ts_sim {
+    Layout L;
+    Ctx ctx;
+    uint8_t* ws = nullptr;
+    cudaStream_t stream = nullptr;
+    int out_on_device = 0;
+    uint32_t k = 0;           // steps enqueued so far
+    int mode = 1;             // 0: two launches per step, 1: persistent cooperative kernel
+    int threads = 256;
+    int grid_persistent = 0, grid_plain = 0;
+    uint32_t sticky = 0;
+};
+
+template <typename T>
+static T* at(ts_sim* s, size_t off) { return reinterpret_cast<T*>(s->ws + off); }
+
+// ------------------------------------------------------------------ kernels
+
+__global__ void __launch_bounds__(256) k_intent(const __grid_constant__ Ctx c, uint32_t k) {
+    phase_intent(c, k, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void __launch_bounds__(256) k_commit(const __grid_constant__ Ctx c, uint32_t k) {
+    phase_commit(c, k, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
+// order-independent digest of state k+1.
+__device__ __forceinline__ void phase_digest(const Ctx& c, unsigned long long* out, uint32_t tid, uint32_t nthreads) {
+    const uint32_t n_slots = __ldcg(&c.dyn->slot_alloc);
+    unsigned long long sum = 0;
+    for (uint32_t s = tid; s < n_slots; s += nthreads) {
+        const uint32_t meta = __ldcg(c.s_meta + s);
+        if (!(meta >> 8)) continue;
+        unsigned long long g = mix64((unsigned long long)__ldcg(c.s_id + s));
+        g = mix64(g ^ (((unsigned long long)__ldcg(c.s_edge + s) << 8) | (meta & 0xFFu)));
+        g = mix64(g ^ (((unsigned long long)__float_as_uint(__ldcg(c.s_x + s)) << 32) |
+                       (unsigned long long)__float_as_uint(__ldcg(c.s_v + s))));
+        sum += g;
+    }
+    if (tid == 0) {
+        unsigned long long g = mix64((unsigned long long)__ldcg(&c.dyn->n_pending));
+        g = mix64(g ^ (unsigned long long)__ldcg(&c.dyn->n_active));
+        g = mix64(g ^ (unsigned long long)__ldcg(&c.dyn->n_arrived));
+        g = mix64(g ^ __ldcg(&c.dyn->sum_arrive));
+        sum += g;
+    }
+    for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+    if ((threadIdx.x & 31) == 0 && sum) atomicAdd(out, sum);
+}
+__global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, unsigned long long* out) {
+    phase_digest(c, out, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
+// n steps in one launch; grid-wide barriers stand where the method has its two dependencies.
+__global__ void __launch_bounds__(256) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
+                                                    unsigned long long* digests) {
+    cg::grid_group grid = cg::this_grid();
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+    for (uint32_t i = 0; i < n; i++) {
+        const uint32_t k = k0 + i;
+        phase_intent(c, k, tid, nthreads);
+        grid.sync();
+        phase_commit(c, k, tid, nthreads);
+        grid.sync();
+        if (digests) phase_digest(c, digests + i, tid, nthreads);
+    }
+}
+
+// State of step 0: every vehicle PENDING.
+__global__ void k_init(const __grid_constant__ Ctx c) {
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+    for (uint32_t i = tid; i < c.V; i += nthreads) {
+        const uint32_t rb = c.route_begin[i];
+        c.o_status[i] = 0; c.o_lane[i] = 0; c.o_edge[i] = c.route_edges[rb]; c.o_x[i] = 0.0f;
+        c.o_v[i] = 0.0f; c.o_rpos[i] = rb; c.o_insert[i] = 0; c.o_arrive[i] = 0;
+    }
+    for (uint32_t q = tid; q < c.n_queues; q += nthreads) { c.queue_head[q] = c.queue_off[q]; c.queue_cand[q] = NONE32; }
+    if (tid == 0) {
+        Dyn d;
+        memset(&d, 0, sizeof d);
+        d.n_pending = c.V;
+        *c.dyn = d;
+    }
+}
+
+// A12 read-back: slot-ordered SoA -> id-ordered arrays.
+__global__ void k_gather_slots(const __grid_constant__ Ctx c) {
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+    const uint32_t n_slots = c.dyn->slot_alloc;
+    for (uint32_t s = tid; s < n_slots; s += nthreads) {
+        const uint32_t meta = c.s_meta[s];
+        if (!(meta >> 8)) continue;
+        const uint32_t id = c.s_id[s];
+        c.o_lane[id] = (uint8_t)(meta & 0xFFu); c.o_edge[id] = c.s_edge[s]; c.o_x[id] = c.s_x[s];
+        c.o_v[id] = c.s_v[s]; c.o_rpos[id] = c.s_rpos[s];
+    }
+}
+__global__ void k_finish_state(const __grid_constant__ Ctx c, uint32_t* o_cell, uint32_t* o_ridx) {
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+    for (uint32_t i = tid; i < c.V; i += nthreads) {
+        o_cell[i] = (uint32_t)floorf(c.o_x[i]);
+        o_ridx[i] = c.o_rpos[i] - c.route_begin[i];
+    }
+}
+
+// ------------------------------------------------------------------ create / reset
+
+static int validate(const ts_network* net, const ts_routes* rt, const ts_departures* dep, const ts_params* p) {
+    if (!dep || !p || !dep->depart_time_s) return fail(TS_EINVAL, "null argument");
+    if (!(p->dt > 0) || !(p->a > 0) || !(p->b > 0) || !(p->T >= 0) || !(p->s0 >= 0))
+        return fail(TS_EINVAL, "params: dt, a, b must be > 0 and T, s0 >= 0");
+    if (!(p->veh_len >= 2.0f)) return fail(TS_EINVAL, "params: veh_len must be >= 2 m");
+    if (p->lookahead_cells < 16 || p->lookahead_cells > 4096 || p->lookahead_cells % 16)
+        return fail(TS_EINVAL, "params: lookahead_cells must be a multiple of 16 in 16..4096");
+    if (p->lookback_cells > 4096) return fail(TS_EINVAL, "params: lookback_cells > 4096");
+    if (p->insert_clear_cells < 1 || p->insert_clear_cells > 16)
+        return fail(TS_EINVAL, "params: insert_clear_cells must be in 1..16");
+    const uint32_t V = rt->n_vehicles, E = net->n_edges, N = net->n_nodes;
+    float max_mult = 1.0f;
+    for (uint32_t i = 0; i < V; i++) {
+        if (dep->v0_mult) {
+            if (!(dep->v0_mult[i] > 0)) return fail(TS_EINVAL, "vehicle %u: v0_mult must be > 0", i);
+            max_mult = std::max(max_mult, dep->v0_mult[i]);
+        }
+        if (!(dep->depart_time_s[i] >= 0)) return fail(TS_EINVAL, "vehicle %u: negative departure time", i);
+        if (std::ceil((double)dep->depart_time_s[i] / (double)p->dt) >= 2147483648.0)
+            return fail(TS_EINVAL, "vehicle %u: departure step beyond 2^31", i);
+    }
+    for (uint32_t e = 0; e < E; e++) {
+        if (net->edge_from[e] >= N || net->edge_to[e] >= N) return fail(TS_EINVAL, "edge %u: endpoint out of range", e);
+        if (!(net->edge_vlim[e] > 0)) return fail(TS_EINVAL, "edge %u: speed limit must be > 0", e);
+        // a vehicle entering an edge must land short of the zone where lanes may be changed (R14)
+        double adv = (double)net->edge_vlim[e] * max_mult * p->dt + 0.5 * p->a * p->dt * p->dt + p->veh_len;
+        if (!(adv < (double)p->entry_zone_cells))
+            return fail(TS_EINVAL, "edge %u: entry_zone_cells %u too short for the fastest vehicle (%.2f m)", e, p->entry_zone_cells, adv);
+    }
+    for (uint32_t h = 0; h < N; h++) {
+        if (net->node_ctrl[h] > 2) return fail(TS_EINVAL, "node %u: unknown control type", h);
+        if (net->node_ctrl[h] == TS_CTRL_SIGNAL) {
+            if (net->sig_green_steps[h] < 1) return fail(TS_EINVAL, "node %u: green must be >= 1 step", h);
+            if ((uint64_t)net->sig_green_steps[h] + net->sig_allred_steps[h] > 65535)
+                return fail(TS_EINVAL, "node %u: green + all-red > 65535 steps", h);
+            if (net->sig_offset_steps[h] >= 0x80000000u) return fail(TS_EINVAL, "node %u: offset >= 2^31", h);
+        }
+    }
+    for (uint32_t i = 0; i < V; i++)
+        for (uint64_t j = rt->route_off[i]; j < rt->route_off[i + 1]; j++) {
+            if (rt->route_edges[j] >= E) return fail(TS_EINVAL, "vehicle %u: route edge out of range", i);
+            if (j > rt->route_off[i] && net->edge_to[rt->route_edges[j - 1]] != net->edge_from[rt->route_edges[j]])
+                return fail(TS_EINVAL, "vehicle %u: route is not contiguous at position %llu", i,
+                            (unsigned long long)(j - rt->route_off[i]));
+        }
+    return TS_OK;
+}
+
+static void bind_ctx(ts_sim* s, const ts_params* p) {
+    Layout& L = s->L;
+    Ctx& c = s->ctx;
+    Params& q = c.p;
+    q.dt = p->dt; q.a = p->a; q.b = p->b; q.T = p->T; q.s0 = p->s0; q.len = p->veh_len;
+    q.b_safe = p->b_safe; q.politeness = p->politeness; q.lc_threshold = p->lc_threshold;
+    { volatile float ab = p->a * p->b; volatile float r = sqrtf(ab); q.K = 2.0f * r; }
+    { volatile float h = 0.5f * p->a; q.half_a_dt = h * p->dt; }
+    q.a_dt = p->a * p->dt;
+    q.entry_zone_f = (float)p->entry_zone_cells;
+    q.H = (int)p->lookahead_cells; q.Hb = (int)p->lookback_cells;
+    q.lc_period = p->lc_period; q.insert_clear = p->insert_clear_cells; q.sample_period = p->sample_period_steps;
+    c.V = L.V; c.E = L.E; c.N = L.N; c.n_queues = L.Q; c.cap_slots = L.cap;
+    c.edges = at<EdgeRec>(s, L.edges); c.route_edges = at<uint32_t>(s, L.route_edges);
+    c.route_begin = at<uint32_t>(s, L.route_begin); c.route_end = at<uint32_t>(s, L.route_end);
+    c.v0_mult = at<float>(s, L.v0_mult); c.mand_dist = at<float>(s, L.mand_dist);
+    c.queue_edge = at<uint32_t>(s, L.queue_edge); c.queue_off = at<uint32_t>(s, L.queue_off);
+    c.queue_veh = at<uint32_t>(s, L.queue_veh); c.queue_dep = at<uint32_t>(s, L.queue_dep);
+    c.atlas = at<uint8_t>(s, L.atlas); c.queue_head = at<uint32_t>(s, L.queue_head);
+    c.queue_cand = at<uint32_t>(s, L.queue_cand);
+    c.lane_claim = at<unsigned long long>(s, L.lane_claim); c.node_claim = at<unsigned long long>(s, L.node_claim);
+    c.dyn = at<Dyn>(s, L.dyn);
+    uint32_t* sl = at<uint32_t>(s, L.slots);
+    size_t cap = L.cap;
+    c.s_x = (float*)(sl + 0 * cap); c.s_v = (float*)(sl + 1 * cap); c.s_edge = sl + 2 * cap; c.s_meta = sl + 3 * cap;
+    c.s_id = sl + 4 * cap; c.s_next = sl + 5 * cap; c.s_rpos = sl + 6 * cap; c.s_enter = sl + 7 * cap;
+    c.s_v0m = (float*)(sl + 8 * cap); c.s_mand = (float*)(sl + 9 * cap);
+    c.s_xt = (float*)(sl + 10 * cap); c.s_vt = (float*)(sl + 11 * cap); c.s_act = sl + 12 * cap;
+    c.o_status = at<uint8_t>(s, L.o_status); c.o_lane = at<uint8_t>(s, L.o_lane);
+    c.o_edge = at<uint32_t>(s, L.o_edge); c.o_x = at<float>(s, L.o_x); c.o_v = at<float>(s, L.o_v);
+    c.o_rpos = at<uint32_t>(s, L.o_rpos); c.o_insert = at<uint32_t>(s, L.o_insert); c.o_arrive = at<uint32_t>(s, L.o_arrive);
+    c.st_entered = at<uint32_t>(s, L.st_entered); c.st_exited = at<uint32_t>(s, L.st_exited);
+    c.st_exit_steps = at<unsigned long long>(s, L.st_exit_steps); c.st_samp_cnt = at<uint32_t>(s, L.st_samp_cnt);
+    c.st_samp_code = at<unsigned long long>(s, L.st_samp_code);
+}
+
+extern "C" int ts_reset(ts_sim* s) {
+    if (!s) return fail(TS_EINVAL, "null sim");
+    Layout& L = s->L;
+    cudaStream_t st = s->stream;
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.atlas, 0, L.atlas_bytes, st));
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.lane_claim, 0xFF, L.n_lanes * 8, st));
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.node_claim, 0xFF, (size_t)L.N * 8, st));
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, st));
+    k_init<<<std::max(1u, std::min(1184u, (L.V + 255) / 256)), 256, 0, st>>>(s->ctx);
+    CUDA_TRY(cudaGetLastError());
+    s->k = 0; s->sticky = 0;
+    return TS_OK;
+}
+
+extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_departures* dep,
+                         const ts_params* p, const ts_device* dev, ts_sim** out) {
+    if (out) *out = nullptr;
+    if (!out || !dev) return fail(TS_EINVAL, "null argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(TS_ECUDA, "no CUDA device: this library has no CPU fallback");
+    Layout L;
+    int rc = plan_sizes(net, rt, L);
+    if (rc) return rc;
+    if ((rc = validate(net, rt, dep, p))) return rc;
+    if (!dev->workspace || ((uintptr_t)dev->workspace & 255)) return fail(TS_EINVAL, "workspace must be a 256-byte aligned device pointer");
+    if (dev->bytes < L.total) return fail(TS_ENOMEM, "workspace too small: %zu < %zu bytes", dev->bytes, L.total);
+
+    const uint32_t V = L.V, E = L.E, N = L.N;
+    // per-edge records: atlas row offsets, claim indices, signal plan of the head node
+    std::vector<uint32_t> n_in(N, 0);
+    std::vector<EdgeRec> edges(E);
+    uint64_t row16 = 0, lane_base = 0;
+    for (uint32_t e = 0; e < E; e++) {
+        EdgeRec& r = edges[e];
+        const uint32_t h = net->edge_to[e], ctrl = net->node_ctrl[h];
+        if (n_in[h] >= 255) return fail(TS_EINVAL, "node %u: more than 255 inbound edges", h);
+        r.row16 = (uint32_t)row16; r.lane_base = (uint32_t)lane_base; r.vlim = net->edge_vlim[e];
+        r.to_node = h; r.len = (uint16_t)net->edge_len_m[e];
+        r.lanes_ctrl = (uint8_t)(net->edge_lanes[e] | (ctrl << 4));
+        r.in_rank = (uint8_t)n_in[h]++;
+        r.green = 1; r.P = 1; r.cycle = 1; r.offset = 0;
+        if (ctrl == TS_CTRL_SIGNAL) {
+            r.green = (uint16_t)net->sig_green_steps[h];
+            r.P = (uint16_t)(net->sig_green_steps[h] + net->sig_allred_steps[h]);
+            r.offset = net->sig_offset_steps[h];
+        }
+        row16 += (uint64_t)net->edge_lanes[e] * ((net->edge_len_m[e] + 15) >> 4);
+        lane_base += net->edge_lanes[e];
+    }
+    for (uint32_t e = 0; e < E; e++)
+        if ((edges[e].lanes_ctrl >> 4) == TS_CTRL_SIGNAL) {
+            uint64_t cyc = (uint64_t)n_in[edges[e].to_node] * edges[e].P;
+            edges[e].cycle = (uint32_t)cyc;
+        }
+    // departure queues: per first edge, FIFO by (departure step, id) (R19)
+    std::vector<uint32_t> dep_step(V), route_begin(V), route_end(V), order(V);
+    for (uint32_t i = 0; i < V; i++) {
+        dep_step[i] = (uint32_t)std::ceil((double)dep->depart_time_s[i] / (double)p->dt);
+        route_begin[i] = (uint32_t)rt->route_off[i]; route_end[i] = (uint32_t)rt->route_off[i + 1];
+    }
+    std::iota(order.begin(), order.end(), 0u);
+    const uint32_t* re = rt->route_edges;
+    std::sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) {
+        const uint32_t ex = re[route_begin[x]], ey = re[route_begin[y]];
+        if (ex != ey) return ex < ey;
+        if (dep_step[x] != dep_step[y]) return dep_step[x] < dep_step[y];
+        return x < y;
+    });
+    std::vector<uint32_t> q_edge, q_off, q_dep(V);
+    for (uint32_t n = 0; n < V; n++) {
+        const uint32_t e = re[route_begin[order[n]]];
+        if (n == 0 || e != q_edge.back()) { q_edge.push_back(e); q_off.push_back(n); }
+        q_dep[n] = dep_step[order[n]];
+    }
+    q_off.push_back(V);
+    if (q_edge.size() != L.Q) return fail(TS_EINVAL, "internal: queue count mismatch");
+
+    ts_sim* s = new ts_sim();
+    s->L = L; s->ws = (uint8_t*)dev->workspace; s->stream = (cudaStream_t)dev->cuda_stream;
+    s->out_on_device = dev->out_on_device;
+    bind_ctx(s, p);
+    std::vector<float> ones, mand;
+    const float* v0m = dep->v0_mult;
+    if (!v0m) { ones.assign(V, 1.0f); v0m = ones.data(); }
+    const float* md = dep->mand_dist_m;
+    if (!md) { mand.assign(V, p->mand_dist_default); md = mand.data(); }
+    cudaStream_t st = s->stream;
+    auto up = [&](size_t off, const void* src, size_t bytes) -> cudaError_t {
+        return bytes ? cudaMemcpyAsync(s->ws + off, src, bytes, cudaMemcpyHostToDevice, st) : cudaSuccess;
+    };
+    cudaError_t ce = cudaSuccess;
+    auto chk = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
+    chk(up(L.edges, edges.data(), (size_t)E * sizeof(EdgeRec)));
+    chk(up(L.route_edges, re, L.R * 4));
+    chk(up(L.route_begin, route_begin.data(), (size_t)V * 4));
+    chk(up(L.route_end, route_end.data(), (size_t)V * 4));
+    chk(up(L.v0_mult, v0m, (size_t)V * 4));
+    chk(up(L.mand_dist, md, (size_t)V * 4));
+    chk(up(L.queue_edge, q_edge.data(), (size_t)L.Q * 4));
+    chk(up(L.queue_off, q_off.data(), ((size_t)L.Q + 1) * 4));
+    chk(up(L.queue_veh, order.data(), (size_t)V * 4));
+    chk(up(L.queue_dep, q_dep.data(), (size_t)V * 4));
+    // the staging vectors die with this scope: make sure the copies have left them
+    chk(cudaStreamSynchronize(st));
+    if (ce != cudaSuccess) { delete s; return fail(TS_ECUDA, "upload: %s", cudaGetErrorString(ce)); }
+
+    int dev_id = 0, sms = 0, per_sm = 0;
+    cudaGetDevice(&dev_id);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev_id);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent, s->threads, 0);
+    if (per_sm < 1) { delete s; return fail(TS_ECUDA, "persistent kernel does not fit on an SM"); }
+    s->grid_persistent = sms * std::min(per_sm, 4);
+    s->grid_plain = sms * 4;
+    if ((rc = ts_reset(s))) { delete s; return rc; }
+    *out = s;
+    return TS_OK;
+}
+
+extern "C" void ts_destroy(ts_sim* s) { delete s; }
+
+extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
+    if (!s || !key) return fail(TS_EINVAL, "null argument");
+    if (!strcmp(key, "mode")) {
+        if (value != 0 && value != 1) return fail(TS_EINVAL, "mode must be 0 or 1");
+        s->mode = (int)value;
+    } else if (!strcmp(key, "blocks_per_sm")) {
+        int dev_id = 0, sms = 0, per_sm = 0;
+        cudaGetDevice(&dev_id);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev_id);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent, s->threads, 0);
+        if (value < 1 || value > per_sm) return fail(TS_EINVAL, "blocks_per_sm must be in 1..%d", per_sm);
+        s->grid_persistent = sms * (int)value;
+        s->grid_plain = sms * (int)value;
+    } else return fail(TS_EINVAL, "unknown option '%s'", key);
+    return TS_OK;
+}
+
+// ------------------------------------------------------------------ stepping
+
+static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
+    if ((uint64_t)s->k + n >= 0x7FFFFFFFull) return fail(TS_EINVAL, "step counter would pass 2^31");
+    cudaStream_t st = s->stream;
+    if (s->mode == 1) {
+        uint32_t k0 = s->k;
+        void* args[] = {&s->ctx, &k0, &n, &d_digests};
+        CUDA_TRY(cudaLaunchCooperativeKernel((void*)k_persistent, dim3(s->grid_persistent), dim3(s->threads), args, 0, st));
+    } else {
+        for (uint32_t i = 0; i < n; i++) {
+            k_intent<<<s->grid_plain, s->threads, 0, st>>>(s->ctx, s->k + i);
+            k_commit<<<s->grid_plain, s->threads, 0, st>>>(s->ctx, s->k + i);
+            if (d_digests) k_digest<<<s->grid_plain, s->threads, 0, st>>>(s->ctx, d_digests + i);
+        }
+        CUDA_TRY(cudaGetLastError());
+    }
+    s->k += n;
+    return TS_OK;
+}
+
+extern "C" int ts_step(ts_sim* s, uint32_t n) {
+    if (!s) return fail(TS_EINVAL, "null sim");
+    if (s->sticky) return fail(TS_EINVARIANT, "sticky device error 0x%x", s->sticky);
+    if (n == 0) return TS_OK;
+    return run_steps(s, n, nullptr);
+}
+
+extern "C" int ts_step_digest(ts_sim* s, uint32_t n, uint64_t* digests) {
+    if (!s || !digests) return fail(TS_EINVAL, "null argument");
+    if (s->sticky) return fail(TS_EINVARIANT, "sticky device error 0x%x", s->sticky);
+    cudaStream_t st = s->stream;
+    unsigned long long* scratch = at<unsigned long long>(s, s->L.digest);
+    for (uint32_t done = 0; done < n;) {
+        const uint32_t m = std::min(n - done, Layout::kDigestChunk);
+        unsigned long long* d = s->out_on_device ? (unsigned long long*)digests + done : scratch;
+        CUDA_TRY(cudaMemsetAsync(d, 0, (size_t)m * 8, st));
+        int rc = run_steps(s, m, d);
+        if (rc) return rc;
+        if (!s->out_on_device) {
+            CUDA_TRY(cudaMemcpyAsync(digests + done, scratch, (size_t)m * 8, cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+        }
+        done += m;
+    }
+    return TS_OK;
+}
+
+// ------------------------------------------------------------------ read-back
+
+static int copy_out(ts_sim* s, void* dst, const void* src, size_t bytes) {
+    if (!dst || !bytes) return TS_OK;
+    CUDA_TRY(cudaMemcpyAsync(dst, src, bytes, s->out_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    return TS_OK;
+}
+
+extern "C" int ts_read_state(ts_sim* s, ts_state_out* o) {
+    if (!s || !o) return fail(TS_EINVAL, "null argument");
+    Layout& L = s->L;
+    const size_t V = L.V;
+    const int g = std::max(1, std::min(1184, (int)((V + 255) / 256)));
+    k_gather_slots<<<g, 256, 0, s->stream>>>(s->ctx);
+    k_finish_state<<<g, 256, 0, s->stream>>>(s->ctx, at<uint32_t>(s, L.o_cell), at<uint32_t>(s, L.o_ridx));
+    CUDA_TRY(cudaGetLastError());
+    int rc = 0;
+    if ((rc = copy_out(s, o->status, s->ws + L.o_status, V))) return rc;
+    if ((rc = copy_out(s, o->lane, s->ws + L.o_lane, V))) return rc;
+    if ((rc = copy_out(s, o->edge, s->ws + L.o_edge, V * 4))) return rc;
+    if ((rc = copy_out(s, o->cell, s->ws + L.o_cell, V * 4))) return rc;
+    if ((rc = copy_out(s, o->x, s->ws + L.o_x, V * 4))) return rc;
+    if ((rc = copy_out(s, o->v, s->ws + L.o_v, V * 4))) return rc;
+    if ((rc = copy_out(s, o->route_idx, s->ws + L.o_ridx, V * 4))) return rc;
+    if ((rc = copy_out(s, o->insert_step, s->ws + L.o_insert, V * 4))) return rc;
+    if ((rc = copy_out(s, o->arrive_step, s->ws + L.o_arrive, V * 4))) return rc;
+    Dyn d;
+    CUDA_TRY(cudaMemcpyAsync(&d, s->ws + L.dyn, sizeof d, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    o->step = s->k; o->n_pending = d.n_pending; o->n_active = d.n_active; o->n_arrived = d.n_arrived;
+    o->vehicle_updates = d.updates;
+    if (d.error) { s->sticky = d.error; return fail(TS_EINVARIANT, "device invariant violated (flags 0x%x): %s", d.error,
+                                                   (d.error & ERR_CELL_CLASH) ? "two vehicles scattered to one atlas cell" : "slot overflow"); }
+    return TS_OK;
+}
+
+extern "C" int ts_read_edge_stats(ts_sim* s, ts_edge_stats_out* o, int reset) {
+    if (!s || !o) return fail(TS_EINVAL, "null argument");
+    Layout& L = s->L;
+    const size_t E = L.E;
+    int rc = 0;
+    if ((rc = copy_out(s, o->entered, s->ws + L.st_entered, E * 4))) return rc;
+    if ((rc = copy_out(s, o->exited, s->ws + L.st_exited, E * 4))) return rc;
+    if ((rc = copy_out(s, o->exit_steps_sum, s->ws + L.st_exit_steps, E * 8))) return rc;
+    if ((rc = copy_out(s, o->sample_count_sum, s->ws + L.st_samp_cnt, E * 4))) return rc;
+    if ((rc = copy_out(s, o->sample_speedcode_sum, s->ws + L.st_samp_code, E * 8))) return rc;
+    Dyn d;
+    CUDA_TRY(cudaMemcpyAsync(&d, s->ws + L.dyn, sizeof d, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    o->n_samples = d.n_samples;
+    if (reset) {
+        CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, s->stream));
+        CUDA_TRY(cudaMemsetAsync(s->ws + L.dyn + offsetof(Dyn, n_samples), 0, 4, s->stream));
+    }
+    return TS_OK;
+}
