@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py -- vehicle-updates/s of the traffic microsimulation on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl reference]
+
+A bench "step" is ONE complete simulated run of the workload (ts_reset, then every simulation
+step of the config through ts_step): one pass of the whole hot path (SURVEY.md 8(a) rows
+A1-A11) over one batch of synthetic input.  One vehicle-update = one ACTIVE vehicle advanced
+one simulation step.  `value` is measured with the inputs resident in HBM (CUDA events on the
+launching stream around ts_step); `e2e` goes through the C ABI with host buffers: ts_create
+(validation + H2D of network, routes, departures), ts_step, ts_read_state (D2H).
+
+Multi-GPU: the path does not shard -- replicas only.  Under torchrun every
+rank runs an independent replica of the same workload; no data-path collective exists.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "vehicle_updates_per_sec"
+UNIT = "vehicle-updates/s"
+
+# Algorithmic bytes per vehicle-update:
+#   32 (state read) + 8 (x, v written) + S_own + S_lc + 2 (atlas erase + store)
+# with S_own / S_lc = mean atlas cells scanned per update in the own lane (+ next edge) and in
+# the lane-change target lane, taken from the oracle's work counters for the full run of the
+# config (tests/golden/work_counters.json, written by tests/golden/make_golden.py).
+SCAN_CELLS_FALLBACK = {"cfg1": 87.3 + 12.9, "cfg2": 11.4 + 2.7, "cfg3": 60.0, "cfg5": 30.0}
+
+
+def load_workload(name):
+    from paper_1807_01148_b200 import workload as W
+    if name == "cfg1":
+        return W.config1()
+    if name == "cfg2":
+        return W.config2()
+    if name == "cfg3":
+        return W.config3()
+    if name == "cfg5":
+        return W.config5()
+    if name == "cfg3_small":            # quick functional check, not a reported workload
+        return W.config3(n_vehicles=50_000, steps=7200, grid=64, n_origin_nodes=512,
+                         depart_mean_s=1200.0, depart_sd_s=400.0, name="cfg3_small")
+    raise SystemExit(f"unknown workload {name}")
+
+
+def bytes_per_update(name):
+    path = os.path.join(ROOT, "tests", "golden", "work_counters.json")
+    try:
+        c = json.load(open(path))[name]
+        cells = (c["own_cells"] + c["next_cells"] + c["lc_cells"]) / c["updates"]
+        src = "oracle counters, full run"
+    except Exception:
+        cells = SCAN_CELLS_FALLBACK.get(name.replace("_small", ""), 60.0)
+        src = "estimate"
+    return 32 + 8 + cells + 2, cells, src
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            f = [t.strip() for t in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(bundle, budget_s, chunk=600):
+    """The oracle as it stands, one thread, on a bounded prefix of the workload."""
+    from oracle import Oracle
+    orc = Oracle(bundle)
+    t0 = time.perf_counter()
+    steps = 0
+    while steps < bundle["steps"]:
+        n = min(chunk, bundle["steps"] - steps)
+        orc.step(n)
+        steps += n
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    upd = orc.counters()["updates"]
+    orc.close()
+    return upd, dt, steps
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    bundle = load_workload(args.workload)
+    budget = max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    times, upds, steps = [], [], 0
+    for i in range(args.warmup + args.steps):
+        upd, dt, steps = time_oracle(bundle, budget)
+        if i >= args.warmup:
+            times.append(dt); upds.append(upd)
+    value = sum(upds) / sum(times)
+    sample = f"first {steps} of {bundle['steps']} simulation steps of {bundle['name']} ({upds[-1]} vehicle-updates) per bench step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "config": {"workload": bundle["name"], "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mode", type=int, default=1, help="1 persistent kernel (default), 0 two launches per step")
+    ap.add_argument("--sim-steps", type=int, default=0, help="override the config's simulation steps (diagnostics)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
+
+    import torch
+    import paper_1807_01148_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    bundle = load_workload(args.workload)
+    sim_steps = args.sim_steps or bundle["steps"]
+    stream = torch.cuda.current_stream()
+    sim = pkg.Sim(bundle, f"cuda:{local}", mode=args.mode)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")   # > 126 MB L2
+
+    def one_run():
+        sim.reset()
+        flush.fill_(1)                                   # L2 flush between timed iterations
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        sim.step(sim_steps)                              # the whole hot path, device-resident inputs
+        e1.record(stream)
+        return e0, e1
+
+    for _ in range(args.warmup):
+        one_run()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [one_run() for _ in range(args.steps)]
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = [a.elapsed_time(b) for a, b in evs]
+    counts = sim.read_counts()
+    updates = int(counts["vehicle_updates"])             # per run (reset zeroes it)
+    total_ms = torch.tensor([sum(ms)], dtype=torch.float64, device=f"cuda:{local}")
+    if dist is not None:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_s = float(total_ms.item()) / 1e3
+    value = updates * args.steps * world / total_s
+
+    # end to end through the C ABI with host buffers (pinned where torch can pin them)
+    h2d = sum(int(np.asarray(bundle[k]).nbytes) for k in (
+        "edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim", "node_ctrl", "sig_green_steps",
+        "sig_allred_steps", "sig_offset_steps", "route_off", "route_edges", "depart_time_s", "v0_mult", "mand_dist_m"))
+    V = bundle["n_vehicles"]
+    d2h = V * (1 + 4 + 1 + 4 + 4 + 4 + 4 + 4 + 4) + 64
+    sim.close()
+    del sim
+    pinned = dict(bundle)
+    for k in ("route_edges", "route_off", "depart_time_s", "v0_mult", "mand_dist_m"):
+        t = torch.from_numpy(np.ascontiguousarray(bundle[k]).view(np.uint8)).pin_memory()
+        pinned[k] = t.numpy().view(bundle[k].dtype)
+        pinned["_keep_" + k] = t
+    e2e_ms = []
+    for i in range(1 + max(1, args.steps)):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        s2 = pkg.Sim(pinned, f"cuda:{local}", mode=args.mode)     # ts_query_workspace + ts_create: H2D
+        s2.step(sim_steps)
+        st = s2.read_state()                                       # D2H of the whole state
+        e1.record(stream)
+        torch.cuda.synchronize()
+        if i > 0:
+            e2e_ms.append(e0.elapsed_time(e1))
+        assert int(st["vehicle_updates"]) == updates
+        s2.close()
+    e2e_t = torch.tensor([sum(e2e_ms)], dtype=torch.float64, device=f"cuda:{local}")
+    if dist is not None:
+        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+    e2e_value = updates * len(e2e_ms) * world / (float(e2e_t.item()) / 1e3)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+    bpu, cells, bsrc = bytes_per_update(args.workload)
+    launch_s = (sum(ms) / len(ms)) / 1e3                  # one k_persistent launch per bench step
+    achieved = bpu * updates / launch_s / 1e9
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": float(total_ms.item()) / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": bundle["name"], "vehicles": V, "edges": bundle["n_edges"],
+                   "sim_steps_per_bench_step": sim_steps, "vehicle_updates_per_bench_step": updates,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "step_kernel": "persistent cooperative" if args.mode == 1 else "two launches per sim step",
+                   "l2": "flushed between timed iterations (256 MiB fill) and inputs (routes+atlas) exceed L2"},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": sum(e2e_ms) / len(e2e_ms)},
+        "gpu_launches": args.steps * (1 if args.mode == 1 else 2 * sim_steps),
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "kernel": "k_persistent" if args.mode == 1 else "k_intent+k_commit",
+                     "bytes_per_update": bpu, "scan_cells_per_update": cells, "bytes_source": bsrc,
+                     "us_per_sim_step": 1e6 * launch_s / sim_steps},
+    }
+    if not args.no_cpu_baseline:
+        upd, dt, steps = time_oracle(bundle, 15.0)
+        out["cpu_baseline"] = {"value": upd / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                               "sample": f"first {steps} of {bundle['steps']} simulation steps of {bundle['name']} "
+                                         f"({upd} vehicle-updates, {dt:.1f} s, single thread)"}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -42,7 +42,7 @@ static int fail(int code, const char* fmt, ...) {
 
 extern "C" const char* ts_last_error(void) { return g_err; }
 extern "C" const char* ts_version(void) {
-    return "0.1 (sm_100a, -fmad=false, IEEE div/sqrt, single-buffer atlas, persistent step kernel)";
+    return "0.1 (sm_100a, -fmad=false, IEEE div/sqrt, two-plane atlas, persistent step kernel)";
 }
 
 // ------------------------------------------------------------------ layout
@@ -50,12 +50,12 @@ extern "C" const char* ts_version(void) {
 struct Layout {
     size_t total = 0;
     uint32_t V = 0, E = 0, N = 0, Q = 0, cap = 0;
-    uint64_t R = 0, n_lanes = 0, atlas_bytes = 0;
+    uint64_t R = 0, n_lanes = 0, atlas_chunks = 0;   // chunk = 128 cells of one lane row
     size_t edges, route_edges, route_begin, route_end, v0_mult, mand_dist, queue_edge, queue_off,
-        queue_veh, queue_dep, atlas, queue_head, queue_cand, lane_claim, node_claim, dyn, slots,
+        queue_veh, queue_dep, codes, occ, queue_head, queue_cand, lane_claim, node_claim, dyn, slots,
         o_status, o_lane, o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered,
         st_exited, st_exit_steps, st_samp_cnt, st_samp_code, digest;
-    static constexpr uint32_t kSlotArrays = 13;
+    static constexpr uint32_t kSlotArrays = 15;
     static constexpr uint32_t kDigestChunk = 8192;
     size_t take(size_t bytes) {
         size_t off = total;
@@ -69,7 +69,8 @@ struct Layout {
         v0_mult = take((size_t)V * 4); mand_dist = take((size_t)V * 4);
         queue_edge = take((size_t)Q * 4); queue_off = take(((size_t)Q + 1) * 4);
         queue_veh = take((size_t)V * 4); queue_dep = take((size_t)V * 4);
-        atlas = take(atlas_bytes);
+        codes = take(atlas_chunks * 128);
+        occ = take((atlas_chunks + 2) * 16);          // two spare chunks: load_win never clamps
         queue_head = take((size_t)Q * 4); queue_cand = take((size_t)Q * 4);
         lane_claim = take(n_lanes * 8); node_claim = take((size_t)N * 8);
         dyn = take(sizeof(Dyn));
@@ -93,16 +94,16 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
     L.V = rt->n_vehicles; L.E = net->n_edges; L.N = net->n_nodes;
     L.R = L.V ? rt->route_off[L.V] : 0;
     if (L.R >= 0xFFFFFFFEull) return fail(TS_EINVAL, "route table too long (%llu entries)", (unsigned long long)L.R);
-    uint64_t rows16 = 0, lanes = 0;
+    uint64_t chunks = 0, lanes = 0;
     for (uint32_t e = 0; e < L.E; e++) {
         uint32_t ln = net->edge_lanes[e], len = net->edge_len_m[e];
         if (ln < 1 || ln > 8) return fail(TS_EINVAL, "edge %u: lanes %u not in 1..8", e, ln);
         if (len < 16 || len > 65535) return fail(TS_EINVAL, "edge %u: length %u not in 16..65535", e, len);
-        rows16 += (uint64_t)ln * ((len + 15) >> 4);
+        chunks += (uint64_t)ln * ((len + 127) >> 7);
         lanes += ln;
     }
-    if (rows16 >= 0xFFFFFFFFull) return fail(TS_EINVAL, "atlas larger than 64 GiB");
-    L.atlas_bytes = rows16 * 16; L.n_lanes = lanes;
+    if (chunks >= 0x1FFFFFFFull) return fail(TS_EINVAL, "atlas larger than 64 GiB");
+    L.atlas_chunks = chunks; L.n_lanes = lanes;
     std::vector<uint8_t> is_origin(L.E, 0);
     uint32_t q = 0;
     for (uint32_t i = 0; i < L.V; i++) {
@@ -147,10 +148,10 @@ static T* at(ts_sim* s, size_t off) { return reinterpret_cast<T*>(s->ws + off); 
 
 // ------------------------------------------------------------------ kernels
 
-__global__ void __launch_bounds__(256) k_intent(const __grid_constant__ Ctx c, uint32_t k) {
+__global__ void __launch_bounds__(256, 4) k_intent(const __grid_constant__ Ctx c, uint32_t k) {
     phase_intent(c, k, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
-__global__ void __launch_bounds__(256) k_commit(const __grid_constant__ Ctx c, uint32_t k) {
+__global__ void __launch_bounds__(256, 4) k_commit(const __grid_constant__ Ctx c, uint32_t k) {
     phase_commit(c, k, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
@@ -182,7 +183,7 @@ __global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, u
 }
 
 // n steps in one launch; grid-wide barriers stand where the method has its two dependencies.
-__global__ void __launch_bounds__(256) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
+__global__ void __launch_bounds__(256, 4) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
                                                     unsigned long long* digests) {
     cg::grid_group grid = cg::this_grid();
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
@@ -301,7 +302,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     c.v0_mult = at<float>(s, L.v0_mult); c.mand_dist = at<float>(s, L.mand_dist);
     c.queue_edge = at<uint32_t>(s, L.queue_edge); c.queue_off = at<uint32_t>(s, L.queue_off);
     c.queue_veh = at<uint32_t>(s, L.queue_veh); c.queue_dep = at<uint32_t>(s, L.queue_dep);
-    c.atlas = at<uint8_t>(s, L.atlas); c.queue_head = at<uint32_t>(s, L.queue_head);
+    c.codes = at<uint8_t>(s, L.codes); c.occ = at<uint4>(s, L.occ); c.queue_head = at<uint32_t>(s, L.queue_head);
     c.queue_cand = at<uint32_t>(s, L.queue_cand);
     c.lane_claim = at<unsigned long long>(s, L.lane_claim); c.node_claim = at<unsigned long long>(s, L.node_claim);
     c.dyn = at<Dyn>(s, L.dyn);
@@ -311,6 +312,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     c.s_id = sl + 4 * cap; c.s_next = sl + 5 * cap; c.s_rpos = sl + 6 * cap; c.s_enter = sl + 7 * cap;
     c.s_v0m = (float*)(sl + 8 * cap); c.s_mand = (float*)(sl + 9 * cap);
     c.s_xt = (float*)(sl + 10 * cap); c.s_vt = (float*)(sl + 11 * cap); c.s_act = sl + 12 * cap;
+    c.s_row = sl + 13 * cap; c.s_nrow = sl + 14 * cap;
     c.o_status = at<uint8_t>(s, L.o_status); c.o_lane = at<uint8_t>(s, L.o_lane);
     c.o_edge = at<uint32_t>(s, L.o_edge); c.o_x = at<float>(s, L.o_x); c.o_v = at<float>(s, L.o_v);
     c.o_rpos = at<uint32_t>(s, L.o_rpos); c.o_insert = at<uint32_t>(s, L.o_insert); c.o_arrive = at<uint32_t>(s, L.o_arrive);
@@ -323,7 +325,7 @@ extern "C" int ts_reset(ts_sim* s) {
     if (!s) return fail(TS_EINVAL, "null sim");
     Layout& L = s->L;
     cudaStream_t st = s->stream;
-    CUDA_TRY(cudaMemsetAsync(s->ws + L.atlas, 0, L.atlas_bytes, st));
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.occ, 0, (L.atlas_chunks + 2) * 16, st));   // codes need no clearing
     CUDA_TRY(cudaMemsetAsync(s->ws + L.lane_claim, 0xFF, L.n_lanes * 8, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.node_claim, 0xFF, (size_t)L.N * 8, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, st));
@@ -351,12 +353,12 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     // per-edge records: atlas row offsets, claim indices, signal plan of the head node
     std::vector<uint32_t> n_in(N, 0);
     std::vector<EdgeRec> edges(E);
-    uint64_t row16 = 0, lane_base = 0;
+    uint64_t row = 0, lane_base = 0;
     for (uint32_t e = 0; e < E; e++) {
         EdgeRec& r = edges[e];
         const uint32_t h = net->edge_to[e], ctrl = net->node_ctrl[h];
         if (n_in[h] >= 255) return fail(TS_EINVAL, "node %u: more than 255 inbound edges", h);
-        r.row16 = (uint32_t)row16; r.lane_base = (uint32_t)lane_base; r.vlim = net->edge_vlim[e];
+        r.row = (uint32_t)row; r.lane_base = (uint32_t)lane_base; r.vlim = net->edge_vlim[e];
         r.to_node = h; r.len = (uint16_t)net->edge_len_m[e];
         r.lanes_ctrl = (uint8_t)(net->edge_lanes[e] | (ctrl << 4));
         r.in_rank = (uint8_t)n_in[h]++;
@@ -366,7 +368,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
             r.P = (uint16_t)(net->sig_green_steps[h] + net->sig_allred_steps[h]);
             r.offset = net->sig_offset_steps[h];
         }
-        row16 += (uint64_t)net->edge_lanes[e] * ((net->edge_len_m[e] + 15) >> 4);
+        row += (uint64_t)net->edge_lanes[e] * ((net->edge_len_m[e] + 127) >> 7);
         lane_base += net->edge_lanes[e];
     }
     for (uint32_t e = 0; e < E; e++)

@@ -5,14 +5,22 @@
 // division so that every fp32 expression below is the written sequence of single operations.
 //
 // One simulation step k -> k+1 is two grid-wide phases:
-//   phase_intent : every ACTIVE vehicle reads state k and the traffic atlas M_k (byte scans,
-//                  16-byte vector loads), decides lane change / acceleration / crossing and
-//                  posts step-tagged atomicMin claims; ready departure-queue heads do the same.
+//   phase_intent : every ACTIVE vehicle reads state k and the traffic atlas M_k, decides lane
+//                  change / acceleration / crossing and posts step-tagged atomicMin claims; ready
+//                  departure-queue heads do the same.
 //   -- grid-wide dependency: all claims visible --
 //   phase_commit : claims are resolved (lowest id wins), state k+1 is written, the vehicle's old
-//                  atlas byte is erased and its new one stored (single buffer; race-free by
+//                  atlas cell is vacated and its new one occupied (single buffer; race-free by
 //                  invariant I6), arrivals retire, departures are appended, samples are taken.
 //   -- grid-wide dependency: M_{k+1} complete --
+//
+// The traffic atlas is two planes over the same rows.  A lane row is
+// `stride` chunks of 128 cells (one cell = one metre), zero-padded:
+//   code plane : one byte per cell, the occupant's speed code (valid only where occupied);
+//   occupancy  : one bit per cell, 16 bytes per chunk, so that "check the following bytes" for a
+//                128-cell lookahead is two independent 16-byte loads and an __ffs instead of a
+//                chain of up to nine dependent loads (measured: the step is latency-bound).
+// Vacating a cell clears its bit only; stale code bytes are never read.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -27,7 +35,7 @@ enum : uint32_t { ERR_CELL_CLASH = 1, ERR_SLOTS = 2 };
 // 32 bytes per edge: everything a vehicle needs to know about the edge it is on (or enters),
 // including the signal plan of the node at its head, in two 16-byte loads.
 struct __align__(16) EdgeRec {
-    uint32_t row16;      // atlas offset of lane 0's row, in 16-byte units
+    uint32_t row;        // atlas offset of lane 0's row, in chunks of 128 cells
     uint32_t lane_base;  // global lane index of lane 0 (index of its claim word)
     float vlim;          // m/s
     uint32_t to_node;
@@ -77,7 +85,8 @@ struct Ctx {
     const uint32_t* queue_veh;          // [V] ids ordered by (edge, dep_step, id)
     const uint32_t* queue_dep;          // [V] dep_step in the same order
     // mutable
-    uint8_t* atlas;                     // traffic atlas, one byte per metre of lane
+    uint8_t* codes;                     // traffic atlas, code plane: one byte per metre of lane
+    uint4* occ;                         // traffic atlas, occupancy plane: one bit per metre
     uint32_t* queue_head;               // [Q]
     uint32_t* queue_cand;               // [Q] candidate id of this step or NONE32
     unsigned long long* lane_claim;     // [n_lanes] step-tagged minimum id
@@ -87,7 +96,9 @@ struct Ctx {
     float* s_x; float* s_v; uint32_t* s_edge; uint32_t* s_meta;   // meta: lane | alive << 8
     uint32_t* s_id; uint32_t* s_next; uint32_t* s_rpos; uint32_t* s_enter;
     float* s_v0m; float* s_mand;
+    uint32_t* s_row;                                               // first chunk of the vehicle's lane row
     float* s_xt; float* s_vt; uint32_t* s_act;                     // intent: act | lane_new << 4
+    uint32_t* s_nrow;                                              // intent: lane row after the move
     // id-ordered results
     uint8_t* o_status; uint8_t* o_lane; uint32_t* o_edge; float* o_x; float* o_v;
     uint32_t* o_rpos; uint32_t* o_insert; uint32_t* o_arrive;
@@ -146,58 +157,85 @@ __device__ __forceinline__ EdgeRec load_edge(const EdgeRec* edges, uint32_t e) {
 }
 __device__ __forceinline__ uint32_t edge_lanes(const EdgeRec& e) { return e.lanes_ctrl & 15u; }
 __device__ __forceinline__ uint32_t edge_ctrl(const EdgeRec& e) { return e.lanes_ctrl >> 4; }
-__device__ __forceinline__ uint32_t stride16(const EdgeRec& e) { return ((uint32_t)e.len + 15u) >> 4; }
-__device__ __forceinline__ const uint8_t* lane_row(const uint8_t* atlas, const EdgeRec& e, uint32_t lane) {
-    return atlas + (((size_t)e.row16 + (size_t)lane * stride16(e)) << 4);
-}
+__device__ __forceinline__ uint32_t row_stride(const EdgeRec& e) { return ((uint32_t)e.len + 127u) >> 7; }
+__device__ __forceinline__ uint32_t lane_row(const EdgeRec& e, uint32_t lane) { return e.row + lane * row_stride(e); }
 
 __device__ __forceinline__ unsigned long long claim_word(uint32_t k, uint32_t id) {
     // newer steps compare smaller, so a stale word never beats a live claim and nothing is cleared
     return ((unsigned long long)(0xFFFFFFFFu - k) << 32) | id;
 }
 
-// 16-bit mask of the non-zero bytes of a 16-byte chunk.
-__device__ __forceinline__ uint32_t nz_mask(const uint4& q) {
-    auto m4 = [](uint32_t w) -> uint32_t {
-        uint32_t t = __vcmpne4(w, 0u);               // 0xFF per non-zero byte
-        return (t & 1u) | ((t >> 7) & 2u) | ((t >> 14) & 4u) | ((t >> 21) & 8u);
-    };
-    return m4(q.x) | (m4(q.y) << 4) | (m4(q.z) << 8) | (m4(q.w) << 12);
+// ---- occupancy windows: 256 cells = two 16-byte chunks of one lane row, loaded together ----
+struct Win {
+    uint4 a, b;   // chunk ch and chunk ch+1 (b = 0 past the end of the row)
+    int base;     // cell index of bit 0 of a
+};
+// `row` = first chunk of the lane row, `ch` = first chunk wanted.  Both loads are unconditional:
+// chunk ch+1 may belong to the next row (the plane ends with two spare chunks), callers mask by
+// the last cell of the edge, so no clamping -- and no dependence on the edge record -- is needed.
+__device__ __forceinline__ Win load_win(const uint4* occ, uint32_t row, int ch) {
+    Win w;
+    w.base = ch << 7;
+    w.a = __ldcg(occ + row + ch);
+    w.b = __ldcg(occ + row + ch + 1);
+    return w;
 }
-__device__ __forceinline__ uint32_t chunk_byte(const uint4& q, int b) {
-    uint32_t w = (b & 8) ? ((b & 4) ? q.w : q.z) : ((b & 4) ? q.y : q.x);
-    return (w >> ((b & 3) * 8)) & 0xFFu;
+__device__ __forceinline__ uint32_t win_word(const Win& w, int i) {
+    switch (i) {
+        case 0: return w.a.x; case 1: return w.a.y; case 2: return w.a.z; case 3: return w.a.w;
+        case 4: return w.b.x; case 5: return w.b.y; case 6: return w.b.z; default: return w.b.w;
+    }
 }
-
 // "we check the following bytes in memory": first occupied cell in [from, to]
-// of a lane row, 16 bytes at a time.  Rows are 16-byte aligned and zero-padded to a multiple
-// of 16, so an aligned chunk never leaves the row.  Returns the cell or -1.
-__device__ __forceinline__ int scan_ahead(const uint8_t* row, int from, int to, uint32_t& code) {
-    if (from > to) return -1;
-    const uint4* r = reinterpret_cast<const uint4*>(row);
-    for (int ch = from >> 4, last = to >> 4; ch <= last; ++ch) {
-        uint4 q = __ldcg(r + ch);
-        uint32_t m = nz_mask(q);
-        int base = ch << 4;
-        if (base < from) m &= 0xFFFFu << (from - base);
-        if (base + 15 > to) m &= 0xFFFFu >> (base + 15 - to);
-        if (m) { int b = __ffs((int)m) - 1; code = chunk_byte(q, b); return base + b; }
+// (inclusive, cells of the window), or -1.
+__device__ __forceinline__ int first_occupied(const Win& w, int from, int to) {
+    const int f = from - w.base, t = to - w.base;      // bit indices in [0, 256)
+    if (f > t) return -1;
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+        const int lo = i << 5;
+        uint32_t m = win_word(w, i);
+        if (f > lo) m &= (f - lo >= 32) ? 0u : (0xFFFFFFFFu << (f - lo));
+        if (t < lo + 31) m &= (t < lo) ? 0u : (0xFFFFFFFFu >> (lo + 31 - t));
+        if (m) return w.base + lo + __ffs((int)m) - 1;
     }
     return -1;
 }
-// Last occupied cell in [from, to] (the lag vehicle), scanning backwards.
-__device__ __forceinline__ int scan_behind(const uint8_t* row, int from, int to, uint32_t& code) {
-    if (from > to) return -1;
-    const uint4* r = reinterpret_cast<const uint4*>(row);
-    for (int ch = to >> 4, first = from >> 4; ch >= first; --ch) {
-        uint4 q = __ldcg(r + ch);
-        uint32_t m = nz_mask(q);
-        int base = ch << 4;
-        if (base < from) m &= 0xFFFFu << (from - base);
-        if (base + 15 > to) m &= 0xFFFFu >> (base + 15 - to);
-        if (m) { int b = 31 - __clz((int)m); code = chunk_byte(q, b); return base + b; }
+// Last occupied cell in [from, to] (the lag vehicle), or -1.
+__device__ __forceinline__ int last_occupied(const Win& w, int from, int to) {
+    const int f = from - w.base, t = to - w.base;
+    if (f > t) return -1;
+#pragma unroll
+    for (int i = 7; i >= 0; i--) {
+        const int lo = i << 5;
+        uint32_t m = win_word(w, i);
+        if (f > lo) m &= (f - lo >= 32) ? 0u : (0xFFFFFFFFu << (f - lo));
+        if (t < lo + 31) m &= (t < lo) ? 0u : (0xFFFFFFFFu >> (lo + 31 - t));
+        if (m) return w.base + lo + 31 - __clz((int)m);
     }
     return -1;
+}
+// General ranges (lookahead > 128 cells): window after window.
+__device__ __forceinline__ int scan_ahead(const uint4* occ, uint32_t row, int from, int to) {
+    if (from > to) return -1;
+    for (int ch = from >> 7; ch <= (to >> 7); ch += 2) {
+        const Win w = load_win(occ, row, ch);
+        const int c = first_occupied(w, max(from, w.base), min(to, w.base + 255));
+        if (c >= 0) return c;
+    }
+    return -1;
+}
+__device__ __forceinline__ int scan_behind(const uint4* occ, uint32_t row, int from, int to) {
+    if (from > to) return -1;
+    for (int ch = to >> 7; ch >= (from >> 7); ch -= 2) {
+        const Win w = load_win(occ, row, max(ch - 1, 0));
+        const int c = last_occupied(w, max(from, w.base), min(to, w.base + 255));
+        if (c >= 0) return c;
+    }
+    return -1;
+}
+__device__ __forceinline__ uint32_t code_at(const uint8_t* codes, uint32_t row, int cell) {
+    return __ldcg(codes + ((size_t)row << 7) + cell);
 }
 
 __device__ __forceinline__ unsigned long long mix64(unsigned long long z) {

@@ -1,6 +1,12 @@
 // ts_phases.cuh -- the two phases of one simulation step as __device__ functions, so that the
 // same code runs from the per-phase kernels and from the persistent cooperative kernel.
 // Rule set and notation: DESIGN.md section 2 (steps 2a-2f, 3, 4, 5); citations per block.
+//
+// The step is latency-bound, so each function is written as a short chain
+// of "trips" to L2: every load of a trip is issued before any of them is consumed.
+//   intent : slot state -> edge records + own-lane window -> next-edge / target-lane windows
+//            -> speed codes -> claims (fire and forget)
+//   commit : slot state + intent -> [crossers only: edge records -> claims] -> stores
 #pragma once
 #include "ts_device.cuh"
 
@@ -11,6 +17,7 @@ namespace ts {
 // DESIGN.md 2, step 2: one ACTIVE vehicle, reads state k and atlas M_k only.
 __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint32_t k) {
     const Params& p = c.p;
+    // trip 1: slot state
     const uint32_t meta = __ldcg(c.s_meta + slot);
     if (!(meta >> 8)) return;
     const uint32_t l = meta & 0xFFu;
@@ -18,10 +25,18 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     const uint32_t e = __ldcg(c.s_edge + slot), e2 = __ldcg(c.s_next + slot);
     const uint32_t id = __ldcg(c.s_id + slot);
     const float v0m = __ldcg(c.s_v0m + slot);
-    const EdgeRec E = load_edge(c.edges, e);
+    const uint32_t row = __ldcg(c.s_row + slot);
+    const float mand = __ldcg(c.s_mand + slot);
+    const int ci = (int)floorf(x);
+    const bool fast = p.H <= 128 && p.Hb <= 128;      // one 256-cell window covers a scan
+
+    // trip 2: edge records and the own-lane window
     const bool last = (e2 == NONE32);
+    const EdgeRec E = load_edge(c.edges, e);
     EdgeRec E2 = E;
     if (!last) E2 = load_edge(c.edges, e2);
+    Win w_own;
+    if (fast) w_own = load_win(c.occ, row, (ci + 1) >> 7);
 
     // 2a
     const float v0 = v0m * E.vlim;
@@ -31,43 +46,15 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     const uint32_t l2 = l < lanes2 - 1 ? l : lanes2 - 1;
     const uint32_t ctrl = edge_ctrl(E);
     const bool may_cross = last || ctrl != CTRL_SIGNAL || signal_green(E, k);
-    const int ci = (int)floorf(x);
-    const uint8_t* row = lane_row(c.atlas, E, l);
+    const int lim = min(C - 1, ci + p.H);
+    const int Hp = p.H - (C - 1 - ci);
+    const bool want_next = !last && may_cross && Hp > 0;
+    const int lim2 = min((int)E2.len - 1, Hp - 1);
+    const uint32_t row2 = lane_row(E2, l2);
 
-    // 2b own leader: first occupied byte after the vehicle's own, at most H cells
-    // ahead, continuing into the target lane of the next route edge if allowed to cross.
-    bool has_lead = false, lead_on_edge = false;
-    float s_lead = 0.0f, dv_lead = 0.0f;
-    {
-        uint32_t code;
-        const int lim = min(C - 1, ci + p.H);
-        int cL = scan_ahead(row, ci + 1, lim, code);
-        if (cL >= 0) {
-            has_lead = lead_on_edge = true;
-            s_lead = (float)cL - p.len;
-            s_lead = s_lead - x;
-            dv_lead = v - speed_decode(code);
-        } else {
-            const int Hp = p.H - (C - 1 - ci);
-            if (!last && may_cross && Hp > 0) {
-                const int lim2 = min((int)E2.len - 1, Hp - 1);
-                int cL2 = scan_ahead(lane_row(c.atlas, E2, l2), 0, lim2, code);
-                if (cL2 >= 0) {
-                    has_lead = true;
-                    s_lead = Cf - x;
-                    s_lead = s_lead + (float)cL2;
-                    s_lead = s_lead - p.len;
-                    dv_lead = v - speed_decode(code);
-                }
-            }
-        }
-    }
-
-    // 2d lane change: staggered evaluation, gap acceptance G1-G3, then the
-    // mandatory rule or the MOBIL incentive (G4).
-    bool accepted = false, has_Lt = false;
-    float s_Lt = 0.0f, at_c = 0.0f;
-    uint32_t lt = l;
+    // 2d eligibility (readings R12, R14): known before any target-lane byte is read
+    bool lc_eval = false;
+    uint32_t lt = l, rowt = row;
     if (p.lc_period != 0 && lanes >= 2) {
         const int lti = (int)l + ((k & 1u) ? -1 : +1);
         float n = v + p.a_dt;
@@ -75,47 +62,86 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
         n = x + n;
         if (lti >= 0 && lti < (int)lanes && x >= p.entry_zone_f && n < Cf &&
             ((k >> 1) + id) % p.lc_period == 0) {
+            lc_eval = true;
             lt = (uint32_t)lti;
-            const uint8_t* rowt = lane_row(c.atlas, E, lt);
-            uint32_t codeL = 1, codeF = 1;
-            const int cLt = scan_ahead(rowt, ci, min(C - 1, ci + p.H), codeL);
-            const int cF = scan_behind(rowt, max(0, ci - p.Hb), ci - 1, codeF);
-            has_Lt = cLt >= 0;
-            const bool has_F = cF >= 0;
-            const float vLt = speed_decode(codeL), vF = speed_decode(codeF);
-            float s_lag = 0.0f;
-            if (has_Lt) { s_Lt = (float)cLt - p.len; s_Lt = s_Lt - x; }
-            if (has_F) { s_lag = x - p.len; s_lag = s_lag - (float)(cF + 1); }
-            bool ok = !has_Lt || s_Lt >= p.s0;                                   // G1
-            float aF_new = 0.0f;
-            if (ok && has_F) {                                                   // G2
-                float m = (vF + 0.125f) + p.half_a_dt;
-                m = m * p.dt;
-                ok = s_lag >= p.s0 && s_lag >= m;
-            }
-            if (ok && has_F) {                                                   // G3
-                aF_new = idm(p, vF, E.vlim, true, s_lag, vF - v);
-                ok = aF_new >= -p.b_safe;
-            }
-            if (ok) {                                                            // G4
-                const float rem = Cf - x;
-                const float mand = __ldcg(c.s_mand + slot);
-                at_c = idm(p, v, v0, has_Lt, s_Lt, v - vLt);
-                if (!last && l >= lanes2 && lt < l && rem <= mand) accepted = true;
-                else if (!last && lt >= lanes2 && rem <= mand) accepted = false;
-                else {
-                    const float a_c = idm(p, v, v0, lead_on_edge, s_lead, dv_lead);
-                    float inc = at_c - a_c;
-                    if (has_F) {
-                        float sF = (float)cLt - p.len;
-                        sF = sF - (float)(cF + 1);
-                        const float a_F = idm(p, vF, E.vlim, has_Lt, sF, vF - vLt);
-                        float d2 = aF_new - a_F;
-                        d2 = p.politeness * d2;
-                        inc = inc + d2;
-                    }
-                    accepted = inc > p.lc_threshold;
+            rowt = lane_row(E, lt);
+        }
+    }
+    const int lo = max(0, ci - p.Hb);
+
+    // trip 3: next-edge window and target-lane windows, all in flight together
+    int cL = -1, cL2 = -1, cLt = -1, cF = -1;
+    if (fast) {
+        Win w_next, w_ta, w_tb;
+        if (want_next) w_next = load_win(c.occ, row2, 0);
+        if (lc_eval) { w_ta = load_win(c.occ, rowt, ci >> 7); w_tb = load_win(c.occ, rowt, lo >> 7); }
+        cL = first_occupied(w_own, ci + 1, lim);                       // 2b
+        if (cL < 0 && want_next) cL2 = first_occupied(w_next, 0, lim2);
+        if (lc_eval) { cLt = first_occupied(w_ta, ci, lim); cF = last_occupied(w_tb, lo, ci - 1); }
+    } else {
+        cL = scan_ahead(c.occ, row, ci + 1, lim);
+        if (cL < 0 && want_next) cL2 = scan_ahead(c.occ, row2, 0, lim2);
+        if (lc_eval) { cLt = scan_ahead(c.occ, rowt, ci, lim); cF = scan_behind(c.occ, rowt, lo, ci - 1); }
+    }
+
+    // trip 4: speed codes of the vehicles found
+    uint32_t code_lead = 1, code_Lt = 1, code_F = 1;
+    if (cL >= 0) code_lead = code_at(c.codes, row, cL);
+    else if (cL2 >= 0) code_lead = code_at(c.codes, row2, cL2);
+    if (cLt >= 0) code_Lt = code_at(c.codes, rowt, cLt);
+    if (cF >= 0) code_F = code_at(c.codes, rowt, cF);
+
+    // 2b gaps (E3)
+    const bool lead_on_edge = cL >= 0, has_lead = cL >= 0 || cL2 >= 0;
+    float s_lead = 0.0f;
+    if (lead_on_edge) {
+        s_lead = (float)cL - p.len;
+        s_lead = s_lead - x;
+    } else if (has_lead) {
+        s_lead = Cf - x;
+        s_lead = s_lead + (float)cL2;
+        s_lead = s_lead - p.len;
+    }
+    const float dv_lead = v - speed_decode(code_lead);
+
+    // 2d gap acceptance G1-G3, then the mandatory rule or the MOBIL incentive G4
+    bool accepted = false;
+    const bool has_Lt = cLt >= 0;
+    float s_Lt = 0.0f, at_c = 0.0f;
+    if (lc_eval) {
+        const bool has_F = cF >= 0;
+        const float vLt = speed_decode(code_Lt), vF = speed_decode(code_F);
+        float s_lag = 0.0f;
+        if (has_Lt) { s_Lt = (float)cLt - p.len; s_Lt = s_Lt - x; }
+        if (has_F) { s_lag = x - p.len; s_lag = s_lag - (float)(cF + 1); }
+        bool ok = !has_Lt || s_Lt >= p.s0;                                   // G1
+        float aF_new = 0.0f;
+        if (ok && has_F) {                                                   // G2 (E4)
+            float m = (vF + 0.125f) + p.half_a_dt;
+            m = m * p.dt;
+            ok = s_lag >= p.s0 && s_lag >= m;
+        }
+        if (ok && has_F) {                                                   // G3
+            aF_new = idm(p, vF, E.vlim, true, s_lag, vF - v);
+            ok = aF_new >= -p.b_safe;
+        }
+        if (ok) {                                                            // G4
+            const float rem = Cf - x;
+            at_c = idm(p, v, v0, has_Lt, s_Lt, v - vLt);
+            if (!last && l >= lanes2 && lt < l && rem <= mand) accepted = true;
+            else if (!last && lt >= lanes2 && rem <= mand) accepted = false;
+            else {
+                const float a_c = idm(p, v, v0, lead_on_edge, s_lead, dv_lead);
+                float inc = at_c - a_c;
+                if (has_F) {
+                    float sF = (float)cLt - p.len;
+                    sF = sF - (float)(cF + 1);
+                    const float a_F = idm(p, vF, E.vlim, has_Lt, sF, vF - vLt);
+                    float d2 = aF_new - a_F;
+                    d2 = p.politeness * d2;
+                    inc = inc + d2;
                 }
+                accepted = inc > p.lc_threshold;
             }
         }
     }
@@ -137,11 +163,12 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     float xt = x + dx;
 
     // 2f crossing intent and claims (one vehicle at a time; lowest id wins)
-    uint32_t act = ACT_STAY;
+    uint32_t act = ACT_STAY, nrow = accepted ? rowt : row;
     if (xt >= Cf) {
         if (last) act = ACT_ARRIVE;
         else if (may_cross) {
             act = ACT_CROSS;
+            nrow = row2;
             const unsigned long long w = claim_word(k, id);
             atomicMin(c.lane_claim + E2.lane_base + l2, w);
             if (ctrl == CTRL_PRIORITY) atomicMin(c.node_claim + E.to_node, w);
@@ -150,6 +177,7 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     c.s_xt[slot] = xt;
     c.s_vt[slot] = vt;
     c.s_act[slot] = act | ((accepted ? lt : l) << 4);
+    c.s_nrow[slot] = nrow;
 }
 
 // DESIGN.md 2, step 3: the head of one departure queue.
@@ -158,8 +186,8 @@ __device__ __forceinline__ void departure_intent(const Ctx& c, uint32_t q, uint3
     const uint32_t head = __ldcg(c.queue_head + q);
     if (head < __ldg(c.queue_off + q + 1) && __ldg(c.queue_dep + head) <= k) {
         const EdgeRec E = load_edge(c.edges, __ldg(c.queue_edge + q));
-        uint32_t code;
-        if (scan_ahead(lane_row(c.atlas, E, 0), 0, (int)c.p.insert_clear - 1, code) < 0) {
+        const Win w = load_win(c.occ, E.row, 0);
+        if (first_occupied(w, 0, (int)c.p.insert_clear - 1) < 0) {
             cand = __ldg(c.queue_veh + head);
             atomicMin(c.lane_claim + E.lane_base, claim_word(k, cand));
         }
@@ -180,79 +208,91 @@ __device__ __forceinline__ void phase_intent(const Ctx& c, uint32_t k, uint32_t 
 
 // ------------------------------------------------------------------ phase 2: resolve + commit
 
-__device__ __forceinline__ void atlas_move(const Ctx& c, uint8_t* from, uint8_t* to, uint32_t code) {
-    // single-buffer erase-then-write: no other vehicle's new cell equals this vehicle's old
-    // cell (invariant I6), so the plain byte stores of different threads never collide.
-    if (from != to) {
-        if (from) *from = 0;
-        if (__ldcg(to) != 0) atomicOr(&c.dyn->error, ERR_CELL_CLASH);
+// Vacate (row_from, cell_from) and occupy (row_to, cell_to) with `code`.  Single buffer: no other
+// vehicle's new cell equals this vehicle's old cell (invariant I6), and bit updates commute, so
+// the integer atomics of different threads never conflict.  The bit that is already set when a
+// cell is occupied is the by-product that proves invariant I2 on the device.
+__device__ __forceinline__ void atlas_move(const Ctx& c, bool has_from, uint32_t row_from, int cell_from,
+                                           uint32_t row_to, int cell_to, uint32_t code) {
+    uint32_t* occ32 = reinterpret_cast<uint32_t*>(c.occ);
+    if (!has_from || row_from != row_to || cell_from != cell_to) {
+        if (has_from) atomicAnd(occ32 + ((size_t)row_from << 2) + (cell_from >> 5), ~(1u << (cell_from & 31)));
+        const uint32_t bit = 1u << (cell_to & 31);
+        const uint32_t old = atomicOr(occ32 + ((size_t)row_to << 2) + (cell_to >> 5), bit);
+        if (old & bit) atomicOr(&c.dyn->error, ERR_CELL_CLASH);
     }
-    *to = (uint8_t)code;
+    c.codes[((size_t)row_to << 7) + cell_to] = (uint8_t)code;
 }
 
 __device__ __forceinline__ void vehicle_commit(const Ctx& c, uint32_t slot, uint32_t k, bool sample) {
+    // trip 1: slot state and intent
     const uint32_t meta = __ldcg(c.s_meta + slot);
     if (!(meta >> 8)) return;
     const uint32_t l = meta & 0xFFu;
     const uint32_t a = __ldcg(c.s_act + slot);
-    const uint32_t act = a & 15u, ln = a >> 4;
     const uint32_t e = __ldcg(c.s_edge + slot);
     const float x_old = __ldcg(c.s_x + slot);
     float xn = __ldcg(c.s_xt + slot), vn = __ldcg(c.s_vt + slot);
-    const EdgeRec E = load_edge(c.edges, e);
+    const uint32_t row = __ldcg(c.s_row + slot);
+    uint32_t nrow = __ldcg(c.s_nrow + slot);
+    const uint32_t act = a & 15u;
+    uint32_t l_new = a >> 4, e_new = e;
     const uint32_t k1 = k + 1;
-    uint8_t* old_cell = const_cast<uint8_t*>(lane_row(c.atlas, E, l)) + (int)floorf(x_old);
-    uint32_t e_new = e, l_new = ln;
-    const uint8_t* new_row = nullptr;
+    const int c_old = (int)floorf(x_old);
 
-    if (act == ACT_CROSS) {
+    if (act != ACT_STAY) {
         const uint32_t id = __ldcg(c.s_id + slot);
         const uint32_t e2 = __ldcg(c.s_next + slot);
-        const EdgeRec E2 = load_edge(c.edges, e2);
-        const uint32_t lanes2 = edge_lanes(E2);
-        const uint32_t l2 = l < lanes2 - 1 ? l : lanes2 - 1;
-        const unsigned long long w = claim_word(k, id);
-        bool win = __ldcg(c.lane_claim + E2.lane_base + l2) == w;
-        if (win && edge_ctrl(E) == CTRL_PRIORITY) win = __ldcg(c.node_claim + E.to_node) == w;
-        const float Cf = (float)E.len;
-        if (win) {
-            xn = xn - Cf;
-            xn = fminf(xn, (float)E2.len - 0.0625f);
-            vn = fminf(vn, __ldcg(c.s_v0m + slot) * E2.vlim);
-            e_new = e2; l_new = l2;
-            new_row = lane_row(c.atlas, E2, l2);
-            const uint32_t rpos = __ldcg(c.s_rpos + slot) + 1;
-            c.s_rpos[slot] = rpos;
-            c.s_next[slot] = (rpos + 1 < __ldg(c.route_end + id)) ? __ldg(c.route_edges + rpos + 1) : NONE32;
-            c.s_edge[slot] = e2;
-            atomicAdd(c.st_entered + e2, 1u);
+        const uint32_t enter = __ldcg(c.s_enter + slot);
+        const uint32_t rpos = __ldcg(c.s_rpos + slot);
+        const EdgeRec E = load_edge(c.edges, e);
+        if (act == ACT_CROSS) {
+            // trip 2: edge records and the route two edges ahead; trip 3: the claim words
+            const EdgeRec E2 = load_edge(c.edges, e2);
+            const uint32_t rend = __ldg(c.route_end + id);
+            const uint32_t e3 = (rpos + 2 < rend) ? __ldg(c.route_edges + rpos + 2) : NONE32;
+            const float v0m = __ldcg(c.s_v0m + slot);
+            const uint32_t lanes2 = edge_lanes(E2);
+            const uint32_t l2 = l < lanes2 - 1 ? l : lanes2 - 1;
+            const unsigned long long w = claim_word(k, id);
+            const unsigned long long wl = __ldcg(c.lane_claim + E2.lane_base + l2);
+            const unsigned long long wn = (edge_ctrl(E) == CTRL_PRIORITY) ? __ldcg(c.node_claim + E.to_node) : w;
+            const float Cf = (float)E.len;
+            if (wl == w && wn == w) {                  // holds every claim it made: crosses
+                xn = xn - Cf;
+                xn = fminf(xn, (float)E2.len - 0.0625f);
+                vn = fminf(vn, v0m * E2.vlim);         // R9
+                e_new = e2; l_new = l2;
+                c.s_rpos[slot] = rpos + 1;
+                c.s_next[slot] = e3;
+                c.s_edge[slot] = e2;
+                c.s_enter[slot] = k1;
+                atomicAdd(c.st_entered + e2, 1u);
+                atomicAdd(c.st_exited + e, 1u);
+                atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - enter));
+            } else {                                   // lost a claim: held at the line (R15)
+                xn = Cf - 0.0625f; vn = 0.0f; l_new = l; nrow = row;
+            }
+        } else {                                       // ACT_ARRIVE
+            atomicAnd(reinterpret_cast<uint32_t*>(c.occ) + ((size_t)row << 2) + (c_old >> 5), ~(1u << (c_old & 31)));
+            c.s_meta[slot] = l;                        // alive bit off
+            c.o_status[id] = 2; c.o_arrive[id] = k1; c.o_x[id] = (float)E.len; c.o_v[id] = vn;
+            c.o_edge[id] = e; c.o_lane[id] = (uint8_t)l; c.o_rpos[id] = rpos;
             atomicAdd(c.st_exited + e, 1u);
-            atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - __ldcg(c.s_enter + slot)));
-            c.s_enter[slot] = k1;
-        } else {                                   // lost a claim: held at the line (R15)
-            xn = Cf - 0.0625f; vn = 0.0f; l_new = l;
+            atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - enter));
+            atomicSub(&c.dyn->n_active, 1u);
+            atomicAdd(&c.dyn->n_arrived, 1u);
+            atomicAdd(&c.dyn->sum_arrive, (unsigned long long)k1);
+            return;
         }
-    } else if (act == ACT_ARRIVE) {
-        const uint32_t id = __ldcg(c.s_id + slot);
-        *old_cell = 0;
-        c.s_meta[slot] = l;                        // alive bit off
-        c.o_status[id] = 2; c.o_arrive[id] = k1; c.o_x[id] = (float)E.len; c.o_v[id] = vn;
-        c.o_edge[id] = e; c.o_lane[id] = (uint8_t)l; c.o_rpos[id] = __ldcg(c.s_rpos + slot);
-        atomicAdd(c.st_exited + e, 1u);
-        atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - __ldcg(c.s_enter + slot)));
-        atomicSub(&c.dyn->n_active, 1u);
-        atomicAdd(&c.dyn->n_arrived, 1u);
-        atomicAdd(&c.dyn->sum_arrive, (unsigned long long)k1);
-        return;
     }
     c.s_x[slot] = xn;
     c.s_v[slot] = vn;
     if (l_new != l) c.s_meta[slot] = l_new | 0x100u;
+    if (nrow != row) c.s_row[slot] = nrow;
     const uint32_t code = speed_code(vn);
-    if (!new_row) new_row = lane_row(c.atlas, E, l_new);
-    uint8_t* new_cell = const_cast<uint8_t*>(new_row) + (int)floorf(xn);
-    atlas_move(c, old_cell, new_cell, code);
-    if (sample) {                                  // PAPER.md:437 one sample per minute
+    atlas_move(c, true, row, c_old, nrow, (int)floorf(xn), code);
+    if (sample) {                                      // PAPER.md:437 one sample per minute
         atomicAdd(c.st_samp_cnt + e_new, 1u);
         atomicAdd(c.st_samp_code + e_new, (unsigned long long)(code - 1));
     }
@@ -270,12 +310,12 @@ __device__ __forceinline__ void departure_commit(const Ctx& c, uint32_t q, uint3
     const uint32_t k1 = k + 1;
     const uint32_t rb = __ldg(c.route_begin + id);
     c.s_x[slot] = 0.0f; c.s_v[slot] = 0.0f; c.s_edge[slot] = e; c.s_meta[slot] = 0x100u;
-    c.s_id[slot] = id; c.s_rpos[slot] = rb; c.s_enter[slot] = k1;
+    c.s_id[slot] = id; c.s_rpos[slot] = rb; c.s_enter[slot] = k1; c.s_row[slot] = E.row;
     c.s_next[slot] = (rb + 1 < __ldg(c.route_end + id)) ? __ldg(c.route_edges + rb + 1) : NONE32;
     c.s_v0m[slot] = __ldg(c.v0_mult + id); c.s_mand[slot] = __ldg(c.mand_dist + id);
     c.o_status[id] = 1; c.o_insert[id] = k1;
     c.queue_head[q] = __ldcg(c.queue_head + q) + 1;
-    atlas_move(c, nullptr, const_cast<uint8_t*>(lane_row(c.atlas, E, 0)), 1u);
+    atlas_move(c, false, 0, 0, E.row, 0, 1u);
     atomicAdd(c.st_entered + e, 1u);
     atomicSub(&c.dyn->n_pending, 1u);
     atomicAdd(&c.dyn->n_active, 1u);
