@@ -35,30 +35,22 @@ UNIT = "vehicle-updates/s"
 #   32 (state read) + 8 (x, v written) + S_own + S_lc + 2 (atlas erase + store)
 # with S_own / S_lc = mean atlas cells scanned per update in the own lane (+ next edge) and in
 # the lane-change target lane, taken from the oracle's work counters for the full run of the
-# config (tests/golden/work_counters.json, written by tests/golden/make_golden.py).
+# config (tests/golden/trace_<cfg>.json, written by tests/golden/make_golden.py).
 SCAN_CELLS_FALLBACK = {"cfg1": 87.3 + 12.9, "cfg2": 11.4 + 2.7, "cfg3": 60.0, "cfg5": 30.0}
 
 
 def load_workload(name):
     from paper_1807_01148_b200 import workload as W
-    if name == "cfg1":
-        return W.config1()
-    if name == "cfg2":
-        return W.config2()
-    if name == "cfg3":
-        return W.config3()
-    if name == "cfg5":
-        return W.config5()
-    if name == "cfg3_small":            # quick functional check, not a reported workload
-        return W.config3(n_vehicles=50_000, steps=7200, grid=64, n_origin_nodes=512,
-                         depart_mean_s=1200.0, depart_sd_s=400.0, name="cfg3_small")
-    raise SystemExit(f"unknown workload {name}")
+    try:
+        return W.by_name(name)
+    except KeyError as e:
+        raise SystemExit(str(e))
 
 
 def bytes_per_update(name):
-    path = os.path.join(ROOT, "tests", "golden", "work_counters.json")
+    path = os.path.join(ROOT, "tests", "golden", f"trace_{name}.json")
     try:
-        c = json.load(open(path))[name]
+        c = json.load(open(path))["counters"]
         cells = (c["own_cells"] + c["next_cells"] + c["lc_cells"]) / c["updates"]
         src = "oracle counters, full run"
     except Exception:
@@ -163,6 +155,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mode", type=int, default=1, help="1 persistent kernel (default), 0 two launches per step")
     ap.add_argument("--sim-steps", type=int, default=0, help="override the config's simulation steps (diagnostics)")
+    ap.add_argument("--start-step", type=int, default=0,
+                    help="advance this many simulation steps untimed before the timed window (diagnostics)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -190,19 +184,26 @@ def main():
         torch.cuda.synchronize()
 
     bundle = load_workload(args.workload)
-    sim_steps = args.sim_steps or bundle["steps"]
+    sim_steps = args.sim_steps or (bundle["steps"] - args.start_step)
     stream = torch.cuda.current_stream()
     sim = pkg.Sim(bundle, f"cuda:{local}", mode=args.mode)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")   # > 126 MB L2
 
     def one_run():
         sim.reset()
+        if args.start_step:
+            sim.set_option("mode", 1)                    # one persistent launch to get there
+            sim.step(args.start_step)                    # untimed: reach the window of interest
+            sim.set_option("mode", args.mode)
+            base = int(sim.read_counts()["vehicle_updates"])
+        else:
+            base = 0
         flush.fill_(1)                                   # L2 flush between timed iterations
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         sim.step(sim_steps)                              # the whole hot path, device-resident inputs
         e1.record(stream)
-        return e0, e1
+        return e0, e1, base
 
     for _ in range(args.warmup):
         one_run()
@@ -213,9 +214,9 @@ def main():
     evs = [one_run() for _ in range(args.steps)]
     barrier()
     clocks = sampler.stop() if rank == 0 else None
-    ms = [a.elapsed_time(b) for a, b in evs]
+    ms = [a.elapsed_time(b) for a, b, _ in evs]
     counts = sim.read_counts()
-    updates = int(counts["vehicle_updates"])             # per run (reset zeroes it)
+    updates = int(counts["vehicle_updates"]) - evs[-1][2]   # per timed window (reset zeroes the counter)
     total_ms = torch.tensor([sum(ms)], dtype=torch.float64, device=f"cuda:{local}")
     if dist is not None:
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
@@ -236,7 +237,7 @@ def main():
         pinned[k] = t.numpy().view(bundle[k].dtype)
         pinned["_keep_" + k] = t
     e2e_ms = []
-    for i in range(1 + max(1, args.steps)):
+    for i in range(0 if args.start_step else 1 + max(1, args.steps)):   # diagnostics windows have no e2e leg
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -252,7 +253,7 @@ def main():
     e2e_t = torch.tensor([sum(e2e_ms)], dtype=torch.float64, device=f"cuda:{local}")
     if dist is not None:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
-    e2e_value = updates * len(e2e_ms) * world / (float(e2e_t.item()) / 1e3)
+    e2e_value = updates * len(e2e_ms) * world / (float(e2e_t.item()) / 1e3) if e2e_ms else None
 
     if rank != 0:
         if dist is not None:
@@ -274,11 +275,12 @@ def main():
         "data": "synthetic",
         "config": {"workload": bundle["name"], "vehicles": V, "edges": bundle["n_edges"],
                    "sim_steps_per_bench_step": sim_steps, "vehicle_updates_per_bench_step": updates,
+                   "start_step": args.start_step,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "step_kernel": "persistent cooperative" if args.mode == 1 else "two launches per sim step",
                    "l2": "flushed between timed iterations (256 MiB fill) and inputs (routes+atlas) exceed L2"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": sum(e2e_ms) / len(e2e_ms)},
+                "ms_per_step": sum(e2e_ms) / len(e2e_ms) if e2e_ms else None},
         "gpu_launches": args.steps * (1 if args.mode == 1 else 2 * sim_steps),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",

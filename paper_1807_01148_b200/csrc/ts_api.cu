@@ -19,6 +19,7 @@
 
 #include "../../include/trafficsim.h"
 #include "ts_phases.cuh"
+#include "ts_sort.cuh"
 
 namespace cg = cooperative_groups;
 using namespace ts;
@@ -42,7 +43,7 @@ static int fail(int code, const char* fmt, ...) {
 
 extern "C" const char* ts_last_error(void) { return g_err; }
 extern "C" const char* ts_version(void) {
-    return "0.1 (sm_100a, -fmad=false, IEEE div/sqrt, two-plane atlas, persistent step kernel)";
+    return "0.2 (sm_100a, -fmad=false, IEEE div/sqrt, two-plane atlas, persistent step kernel, edge-sorted slots)";
 }
 
 // ------------------------------------------------------------------ layout
@@ -51,11 +52,10 @@ struct Layout {
     size_t total = 0;
     uint32_t V = 0, E = 0, N = 0, Q = 0, cap = 0;
     uint64_t R = 0, n_lanes = 0, atlas_chunks = 0;   // chunk = 128 cells of one lane row
-    size_t edges, route_edges, route_begin, route_end, v0_mult, mand_dist, queue_edge, queue_off,
-        queue_veh, queue_dep, codes, occ, queue_head, queue_cand, lane_claim, node_claim, dyn, slots,
-        o_status, o_lane, o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered,
-        st_exited, st_exit_steps, st_samp_cnt, st_samp_code, digest;
-    static constexpr uint32_t kSlotArrays = 15;
+    size_t edges, route_edges, route_begin, queue_rec, dep_rec, codes, occ, queue_state, queue_cand,
+        lane_claim, node_claim, dyn, barrier, slots, mr_g, cr, rank, hist, base, partial, o_status, o_lane,
+        o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered, st_exited,
+        st_exit_steps, st_samp_cnt, st_samp_code, digest;
     static constexpr uint32_t kDigestChunk = 8192;
     size_t take(size_t bytes) {
         size_t off = total;
@@ -65,16 +65,18 @@ struct Layout {
     void plan() {
         edges = take((size_t)E * sizeof(EdgeRec));
         route_edges = take(R * 4);
-        route_begin = take((size_t)V * 4); route_end = take((size_t)V * 4);
-        v0_mult = take((size_t)V * 4); mand_dist = take((size_t)V * 4);
-        queue_edge = take((size_t)Q * 4); queue_off = take(((size_t)Q + 1) * 4);
-        queue_veh = take((size_t)V * 4); queue_dep = take((size_t)V * 4);
+        route_begin = take((size_t)V * 4);
+        queue_rec = take((size_t)Q * 16);
+        dep_rec = take((size_t)V * 32);
         codes = take(atlas_chunks * 128);
         occ = take((atlas_chunks + 2) * 16);          // two spare chunks: load_win never clamps
-        queue_head = take((size_t)Q * 4); queue_cand = take((size_t)Q * 4);
+        queue_state = take((size_t)Q * 16); queue_cand = take((size_t)Q * 16);
         lane_claim = take(n_lanes * 8); node_claim = take((size_t)N * 8);
-        dyn = take(sizeof(Dyn));
-        slots = take((size_t)cap * 4 * kSlotArrays);
+        dyn = take(sizeof(Dyn)); barrier = take(256);
+        slots = take((size_t)cap * 16 * 6);           // A, B, C in two ping-pong sets
+        mr_g = take((size_t)cap * 16); cr = take((size_t)cap * 32);
+        rank = take((size_t)cap * 4); hist = take((size_t)E * 4); base = take((size_t)E * 4);
+        partial = take((size_t)kMaxCtas * 4);
         o_status = take(V); o_lane = take(V);
         o_edge = take((size_t)V * 4); o_x = take((size_t)V * 4); o_v = take((size_t)V * 4);
         o_rpos = take((size_t)V * 4); o_insert = take((size_t)V * 4); o_arrive = take((size_t)V * 4);
@@ -90,7 +92,7 @@ struct Layout {
 static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
     if (!net || !rt) return fail(TS_EINVAL, "null argument");
     if (net->n_edges == 0 || net->n_nodes == 0) return fail(TS_EINVAL, "empty network");
-    if (rt->n_vehicles >= 0xFFFFFFFEu) return fail(TS_EINVAL, "too many vehicles");
+    if (rt->n_vehicles >= 0x7FFFFFF0u) return fail(TS_EINVAL, "too many vehicles");
     L.V = rt->n_vehicles; L.E = net->n_edges; L.N = net->n_nodes;
     L.R = L.V ? rt->route_off[L.V] : 0;
     if (L.R >= 0xFFFFFFFEull) return fail(TS_EINVAL, "route table too long (%llu entries)", (unsigned long long)L.R);
@@ -102,7 +104,8 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
         chunks += (uint64_t)ln * ((len + 127) >> 7);
         lanes += ln;
     }
-    if (chunks >= 0x1FFFFFFFull) return fail(TS_EINVAL, "atlas larger than 64 GiB");
+    // a cell is addressed by one 32-bit index (row * 128 + cell)
+    if (chunks + 2 >= (1ull << 25)) return fail(TS_EINVAL, "atlas larger than 2^32 cells");
     L.atlas_chunks = chunks; L.n_lanes = lanes;
     std::vector<uint8_t> is_origin(L.E, 0);
     uint32_t q = 0;
@@ -112,7 +115,10 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
         if (e >= L.E) return fail(TS_EINVAL, "vehicle %u: route edge %u out of range", i, e);
         if (!is_origin[e]) { is_origin[e] = 1; q++; }
     }
-    L.Q = q; L.cap = L.V;   // every vehicle takes exactly one slot in its life
+    L.Q = q;
+    // a vehicle takes one slot when it departs; a queue head that is ready but has not won its
+    // lane yet holds one reserved slot, which a compaction may drop (then it takes a new one)
+    L.cap = (uint32_t)std::min<uint64_t>((uint64_t)L.V + q + 1024ull, 0x7FFFFFF0ull);
     L.plan();
     return TS_OK;
 }
@@ -137,9 +143,13 @@ struct ts_sim {
     cudaStream_t stream = nullptr;
     int out_on_device = 0;
     uint32_t k = 0;           // steps enqueued so far
-    int mode = 1;             // 0: two launches per step, 1: persistent cooperative kernel
-    int threads = 256;
-    int grid_persistent = 0, grid_plain = 0;
+    uint32_t cur = 0;         // which slot set holds the state
+    int mode = 1;             // 0: one launch per phase, 1: persistent cooperative kernel
+    int threads = 1024;       // persistent kernel CTA size
+    int blocks_per_sm = 1;
+    int sms = 0;
+    uint32_t sort_period = 64;   // steps between compaction + re-sort; 0 = never
+    int smem_limit = 0;
     uint32_t sticky = 0;
 };
 
@@ -148,53 +158,93 @@ static T* at(ts_sim* s, size_t off) { return reinterpret_cast<T*>(s->ws + off); 
 
 // ------------------------------------------------------------------ kernels
 
-__global__ void __launch_bounds__(256, 4) k_intent(const __grid_constant__ Ctx c, uint32_t k) {
-    phase_intent(c, k, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
-}
-__global__ void __launch_bounds__(256, 4) k_commit(const __grid_constant__ Ctx c, uint32_t k) {
-    phase_commit(c, k, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+__device__ __forceinline__ Who who() {
+    Who w;
+    w.t = threadIdx.x; w.T = blockDim.x; w.cta = blockIdx.x; w.n_cta = gridDim.x;
+    return w;
 }
 
-// order-independent digest of state k+1.
-__device__ __forceinline__ void phase_digest(const Ctx& c, unsigned long long* out, uint32_t tid, uint32_t nthreads) {
-    const uint32_t n_slots = __ldcg(&c.dyn->slot_alloc);
-    unsigned long long sum = 0;
-    for (uint32_t s = tid; s < n_slots; s += nthreads) {
-        const uint32_t meta = __ldcg(c.s_meta + s);
-        if (!(meta >> 8)) continue;
-        unsigned long long g = mix64((unsigned long long)__ldcg(c.s_id + s));
-        g = mix64(g ^ (((unsigned long long)__ldcg(c.s_edge + s) << 8) | (meta & 0xFFu)));
-        g = mix64(g ^ (((unsigned long long)__float_as_uint(__ldcg(c.s_x + s)) << 32) |
-                       (unsigned long long)__float_as_uint(__ldcg(c.s_v + s))));
-        sum += g;
+// Grid-wide barrier of the persistent kernel: one arrival per CTA on a monotonic counter.
+// bar.sync orders the CTA's writes before thread 0's release; the acquire load plus the second
+// bar.sync orders them before every later read of any thread (mutable data is read with ld.cg,
+// i.e. from L2, so no stale L1 line can be observed).
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target) {
+    target += gridDim.x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+        unsigned int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+        } while ((int)(v - target) < 0);
     }
-    if (tid == 0) {
-        unsigned long long g = mix64((unsigned long long)__ldcg(&c.dyn->n_pending));
-        g = mix64(g ^ (unsigned long long)__ldcg(&c.dyn->n_active));
-        g = mix64(g ^ (unsigned long long)__ldcg(&c.dyn->n_arrived));
-        g = mix64(g ^ __ldcg(&c.dyn->sum_arrive));
-        sum += g;
-    }
-    for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
-    if ((threadIdx.x & 31) == 0 && sum) atomicAdd(out, sum);
+    __syncthreads();
 }
-__global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, unsigned long long* out) {
-    phase_digest(c, out, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
-}
+
+extern __shared__ uint4 dyn_smem[];
 
 // n steps in one launch; grid-wide barriers stand where the method has its two dependencies.
-__global__ void __launch_bounds__(256, 4) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
-                                                    unsigned long long* digests) {
-    cg::grid_group grid = cg::this_grid();
-    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+__global__ void __launch_bounds__(1024, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
+                                                       uint32_t cur, uint32_t sort_period, uint32_t mr_j,
+                                                       unsigned long long* digests) {
+    __shared__ uint32_t red[33];
+    const Who me = who();
+    unsigned int target = 0;
+    uint32_t n_upd = 0;
     for (uint32_t i = 0; i < n; i++) {
         const uint32_t k = k0 + i;
-        phase_intent(c, k, tid, nthreads);
-        grid.sync();
-        phase_commit(c, k, tid, nthreads);
-        grid.sync();
-        if (digests) phase_digest(c, digests + i, tid, nthreads);
+        const Slots& S = c.s[cur];
+        const uint32_t n_slots = phase1(c, S, k, me, dyn_smem, mr_j, n_upd);
+        grid_barrier(c.barrier, target);
+        phase2(c, S, k, me, dyn_smem, mr_j, n_slots);
+        grid_barrier(c.barrier, target);
+        if (digests) phase_digest(c, S, digests + i, me);
+        if (sort_period && (k + 1) % sort_period == 0) {      // A9 + A10, between two steps
+            const uint32_t ns = sort_rank(c, S, me);
+            grid_barrier(c.barrier, target);
+            sort_partial(c, me, red);
+            grid_barrier(c.barrier, target);
+            sort_scan(c, me, red);
+            grid_barrier(c.barrier, target);
+            sort_scatter(c, S, c.s[cur ^ 1], me, ns);
+            grid_barrier(c.barrier, target);
+            cur ^= 1;
+        }
     }
+    n_upd = block_sum(n_upd, red);
+    if (me.t == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
+}
+
+// The same phases as separate launches (mode 0: profiling per phase, and a fallback where a
+// cooperative launch is not possible).  Move records go through global memory.
+__global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
+    __shared__ uint32_t red[33];
+    uint32_t n_upd = 0;
+    const uint32_t n_slots = phase1(c, c.s[cur], k, who(), nullptr, 0, n_upd);
+    if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n_slots;   // phase 2 overwrites dyn->n_slots
+    n_upd = block_sum(n_upd, red);
+    if (threadIdx.x == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
+}
+__global__ void __launch_bounds__(256) k_phase2(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
+    phase2(c, c.s[cur], k, who(), nullptr, 0, __ldcg(&c.dyn->pad));
+}
+__global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, uint32_t cur, unsigned long long* out) {
+    phase_digest(c, c.s[cur], out, who());
+}
+__global__ void __launch_bounds__(256) k_sort_rank(const __grid_constant__ Ctx c, uint32_t cur) {
+    const uint32_t n = sort_rank(c, c.s[cur], who());
+    if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n;
+}
+__global__ void __launch_bounds__(256) k_sort_partial(const __grid_constant__ Ctx c) {
+    __shared__ uint32_t red[33];
+    sort_partial(c, who(), red);
+}
+__global__ void __launch_bounds__(256) k_sort_scan(const __grid_constant__ Ctx c) {
+    __shared__ uint32_t red[33];
+    sort_scan(c, who(), red);
+}
+__global__ void __launch_bounds__(256) k_sort_scatter(const __grid_constant__ Ctx c, uint32_t cur) {
+    sort_scatter(c, c.s[cur], c.s[cur ^ 1], who(), __ldcg(&c.dyn->pad));
 }
 
 // State of step 0: every vehicle PENDING.
@@ -205,25 +255,31 @@ __global__ void k_init(const __grid_constant__ Ctx c) {
         c.o_status[i] = 0; c.o_lane[i] = 0; c.o_edge[i] = c.route_edges[rb]; c.o_x[i] = 0.0f;
         c.o_v[i] = 0.0f; c.o_rpos[i] = rb; c.o_insert[i] = 0; c.o_arrive[i] = 0;
     }
-    for (uint32_t q = tid; q < c.n_queues; q += nthreads) { c.queue_head[q] = c.queue_off[q]; c.queue_cand[q] = NONE32; }
+    for (uint32_t q = tid; q < c.n_queues; q += nthreads) {
+        const uint32_t head = q ? c.queue_rec[q - 1].z : 0u;        // queues are contiguous in dep_rec
+        c.queue_state[q] = make_uint4(head, c.dep_rec[2 * (size_t)head + 1].z, NONE32, 0);
+        c.queue_cand[q] = make_uint4(NONE32, 0, head, 0);
+    }
     if (tid == 0) {
         Dyn d;
         memset(&d, 0, sizeof d);
-        d.n_pending = c.V;
         *c.dyn = d;
+        *c.barrier = 0;
     }
 }
 
-// A12 read-back: slot-ordered SoA -> id-ordered arrays.
-__global__ void k_gather_slots(const __grid_constant__ Ctx c) {
+// A12 read-back: slot-ordered state -> id-ordered arrays.
+__global__ void k_gather_slots(const __grid_constant__ Ctx c, uint32_t cur) {
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
-    const uint32_t n_slots = c.dyn->slot_alloc;
+    const uint32_t n_slots = min(c.dyn->slot_alloc, c.cap_slots);
+    const Slots& S = c.s[cur];
     for (uint32_t s = tid; s < n_slots; s += nthreads) {
-        const uint32_t meta = c.s_meta[s];
-        if (!(meta >> 8)) continue;
-        const uint32_t id = c.s_id[s];
-        c.o_lane[id] = (uint8_t)(meta & 0xFFu); c.o_edge[id] = c.s_edge[s]; c.o_x[id] = c.s_x[s];
-        c.o_v[id] = c.s_v[s]; c.o_rpos[id] = c.s_rpos[s];
+        const uint4 sa = S.A[s];
+        if (!(sa.w & ALIVE)) continue;
+        const uint4 sb = S.B[s];
+        const uint32_t id = sb.z;
+        c.o_lane[id] = (uint8_t)(sa.w & 0xFu); c.o_edge[id] = sb.x; c.o_x[id] = __uint_as_float(sa.x);
+        c.o_v[id] = __uint_as_float(sa.y); c.o_rpos[id] = S.C[s].x;
     }
 }
 __global__ void k_finish_state(const __grid_constant__ Ctx c, uint32_t* o_cell, uint32_t* o_ridx) {
@@ -298,21 +354,18 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     q.lc_period = p->lc_period; q.insert_clear = p->insert_clear_cells; q.sample_period = p->sample_period_steps;
     c.V = L.V; c.E = L.E; c.N = L.N; c.n_queues = L.Q; c.cap_slots = L.cap;
     c.edges = at<EdgeRec>(s, L.edges); c.route_edges = at<uint32_t>(s, L.route_edges);
-    c.route_begin = at<uint32_t>(s, L.route_begin); c.route_end = at<uint32_t>(s, L.route_end);
-    c.v0_mult = at<float>(s, L.v0_mult); c.mand_dist = at<float>(s, L.mand_dist);
-    c.queue_edge = at<uint32_t>(s, L.queue_edge); c.queue_off = at<uint32_t>(s, L.queue_off);
-    c.queue_veh = at<uint32_t>(s, L.queue_veh); c.queue_dep = at<uint32_t>(s, L.queue_dep);
-    c.codes = at<uint8_t>(s, L.codes); c.occ = at<uint4>(s, L.occ); c.queue_head = at<uint32_t>(s, L.queue_head);
-    c.queue_cand = at<uint32_t>(s, L.queue_cand);
+    c.route_begin = at<uint32_t>(s, L.route_begin);
+    c.queue_rec = at<uint4>(s, L.queue_rec); c.dep_rec = at<uint4>(s, L.dep_rec);
+    c.codes = at<uint8_t>(s, L.codes); c.occ = at<uint4>(s, L.occ);
+    c.queue_state = at<uint4>(s, L.queue_state); c.queue_cand = at<uint4>(s, L.queue_cand);
     c.lane_claim = at<unsigned long long>(s, L.lane_claim); c.node_claim = at<unsigned long long>(s, L.node_claim);
-    c.dyn = at<Dyn>(s, L.dyn);
-    uint32_t* sl = at<uint32_t>(s, L.slots);
-    size_t cap = L.cap;
-    c.s_x = (float*)(sl + 0 * cap); c.s_v = (float*)(sl + 1 * cap); c.s_edge = sl + 2 * cap; c.s_meta = sl + 3 * cap;
-    c.s_id = sl + 4 * cap; c.s_next = sl + 5 * cap; c.s_rpos = sl + 6 * cap; c.s_enter = sl + 7 * cap;
-    c.s_v0m = (float*)(sl + 8 * cap); c.s_mand = (float*)(sl + 9 * cap);
-    c.s_xt = (float*)(sl + 10 * cap); c.s_vt = (float*)(sl + 11 * cap); c.s_act = sl + 12 * cap;
-    c.s_row = sl + 13 * cap; c.s_nrow = sl + 14 * cap;
+    c.dyn = at<Dyn>(s, L.dyn); c.barrier = at<unsigned int>(s, L.barrier);
+    uint4* sl = at<uint4>(s, L.slots);
+    const size_t cap = L.cap;
+    for (int i = 0; i < 2; i++) { c.s[i].A = sl + (3 * i + 0) * cap; c.s[i].B = sl + (3 * i + 1) * cap; c.s[i].C = sl + (3 * i + 2) * cap; }
+    c.mr_g = at<uint4>(s, L.mr_g); c.cr = at<uint4>(s, L.cr);
+    c.rank = at<uint32_t>(s, L.rank); c.hist = at<uint32_t>(s, L.hist); c.base = at<uint32_t>(s, L.base);
+    c.partial = at<uint32_t>(s, L.partial);
     c.o_status = at<uint8_t>(s, L.o_status); c.o_lane = at<uint8_t>(s, L.o_lane);
     c.o_edge = at<uint32_t>(s, L.o_edge); c.o_x = at<float>(s, L.o_x); c.o_v = at<float>(s, L.o_v);
     c.o_rpos = at<uint32_t>(s, L.o_rpos); c.o_insert = at<uint32_t>(s, L.o_insert); c.o_arrive = at<uint32_t>(s, L.o_arrive);
@@ -328,10 +381,11 @@ extern "C" int ts_reset(ts_sim* s) {
     CUDA_TRY(cudaMemsetAsync(s->ws + L.occ, 0, (L.atlas_chunks + 2) * 16, st));   // codes need no clearing
     CUDA_TRY(cudaMemsetAsync(s->ws + L.lane_claim, 0xFF, L.n_lanes * 8, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.node_claim, 0xFF, (size_t)L.N * 8, st));
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.hist, 0, (size_t)L.E * 4, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, st));
     k_init<<<std::max(1u, std::min(1184u, (L.V + 255) / 256)), 256, 0, st>>>(s->ctx);
     CUDA_TRY(cudaGetLastError());
-    s->k = 0; s->sticky = 0;
+    s->k = 0; s->cur = 0; s->sticky = 0;
     return TS_OK;
 }
 
@@ -377,10 +431,10 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
             edges[e].cycle = (uint32_t)cyc;
         }
     // departure queues: per first edge, FIFO by (departure step, id) (R19)
-    std::vector<uint32_t> dep_step(V), route_begin(V), route_end(V), order(V);
+    std::vector<uint32_t> dep_step(V), route_begin(V), order(V);
     for (uint32_t i = 0; i < V; i++) {
         dep_step[i] = (uint32_t)std::ceil((double)dep->depart_time_s[i] / (double)p->dt);
-        route_begin[i] = (uint32_t)rt->route_off[i]; route_end[i] = (uint32_t)rt->route_off[i + 1];
+        route_begin[i] = (uint32_t)rt->route_off[i];
     }
     std::iota(order.begin(), order.end(), 0u);
     const uint32_t* re = rt->route_edges;
@@ -390,24 +444,27 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         if (dep_step[x] != dep_step[y]) return dep_step[x] < dep_step[y];
         return x < y;
     });
-    std::vector<uint32_t> q_edge, q_off, q_dep(V);
+    // one 32-byte departure record per vehicle in queue order, one 16-byte record per queue
+    std::vector<uint4> dep_rec(2 * (size_t)V), queue_rec;
+    auto fbits = [](float f) { uint32_t u; memcpy(&u, &f, 4); return u; };
     for (uint32_t n = 0; n < V; n++) {
-        const uint32_t e = re[route_begin[order[n]]];
-        if (n == 0 || e != q_edge.back()) { q_edge.push_back(e); q_off.push_back(n); }
-        q_dep[n] = dep_step[order[n]];
+        const uint32_t i = order[n], rb = route_begin[i], rend = (uint32_t)rt->route_off[i + 1];
+        const uint32_t e = re[rb];
+        if (n == 0 || e != queue_rec.back().w) {
+            if (!queue_rec.empty()) queue_rec.back().z = n;
+            queue_rec.push_back(make_uint4(edges[e].row, edges[e].lane_base, V, e));
+        }
+        const float v0m = dep->v0_mult ? dep->v0_mult[i] : 1.0f;
+        const float md = dep->mand_dist_m ? dep->mand_dist_m[i] : p->mand_dist_default;
+        dep_rec[2 * (size_t)n] = make_uint4(i, fbits(v0m), fbits(md), rb);
+        dep_rec[2 * (size_t)n + 1] = make_uint4(rend, rb + 1 < rend ? re[rb + 1] : NONE32, dep_step[i], 0);
     }
-    q_off.push_back(V);
-    if (q_edge.size() != L.Q) return fail(TS_EINVAL, "internal: queue count mismatch");
+    if (queue_rec.size() != L.Q) return fail(TS_EINVAL, "internal: queue count mismatch");
 
     ts_sim* s = new ts_sim();
     s->L = L; s->ws = (uint8_t*)dev->workspace; s->stream = (cudaStream_t)dev->cuda_stream;
     s->out_on_device = dev->out_on_device;
     bind_ctx(s, p);
-    std::vector<float> ones, mand;
-    const float* v0m = dep->v0_mult;
-    if (!v0m) { ones.assign(V, 1.0f); v0m = ones.data(); }
-    const float* md = dep->mand_dist_m;
-    if (!md) { mand.assign(V, p->mand_dist_default); md = mand.data(); }
     cudaStream_t st = s->stream;
     auto up = [&](size_t off, const void* src, size_t bytes) -> cudaError_t {
         return bytes ? cudaMemcpyAsync(s->ws + off, src, bytes, cudaMemcpyHostToDevice, st) : cudaSuccess;
@@ -417,24 +474,20 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     chk(up(L.edges, edges.data(), (size_t)E * sizeof(EdgeRec)));
     chk(up(L.route_edges, re, L.R * 4));
     chk(up(L.route_begin, route_begin.data(), (size_t)V * 4));
-    chk(up(L.route_end, route_end.data(), (size_t)V * 4));
-    chk(up(L.v0_mult, v0m, (size_t)V * 4));
-    chk(up(L.mand_dist, md, (size_t)V * 4));
-    chk(up(L.queue_edge, q_edge.data(), (size_t)L.Q * 4));
-    chk(up(L.queue_off, q_off.data(), ((size_t)L.Q + 1) * 4));
-    chk(up(L.queue_veh, order.data(), (size_t)V * 4));
-    chk(up(L.queue_dep, q_dep.data(), (size_t)V * 4));
+    chk(up(L.queue_rec, queue_rec.data(), (size_t)L.Q * 16));
+    chk(up(L.dep_rec, dep_rec.data(), (size_t)V * 32));
     // the staging vectors die with this scope: make sure the copies have left them
     chk(cudaStreamSynchronize(st));
     if (ce != cudaSuccess) { delete s; return fail(TS_ECUDA, "upload: %s", cudaGetErrorString(ce)); }
 
-    int dev_id = 0, sms = 0, per_sm = 0;
+    int dev_id = 0;
     cudaGetDevice(&dev_id);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev_id);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent, s->threads, 0);
-    if (per_sm < 1) { delete s; return fail(TS_ECUDA, "persistent kernel does not fit on an SM"); }
-    s->grid_persistent = sms * std::min(per_sm, 4);
-    s->grid_plain = sms * 4;
+    cudaDeviceGetAttribute(&s->sms, cudaDevAttrMultiProcessorCount, dev_id);
+    cudaDeviceGetAttribute(&s->smem_limit, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_id);
+    if (cudaFuncSetAttribute(k_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess) {
+        delete s;
+        return fail(TS_ECUDA, "cannot raise the dynamic shared memory limit of the step kernel");
+    }
     if ((rc = ts_reset(s))) { delete s; return rc; }
     *out = s;
     return TS_OK;
@@ -448,13 +501,15 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
         if (value != 0 && value != 1) return fail(TS_EINVAL, "mode must be 0 or 1");
         s->mode = (int)value;
     } else if (!strcmp(key, "blocks_per_sm")) {
-        int dev_id = 0, sms = 0, per_sm = 0;
-        cudaGetDevice(&dev_id);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev_id);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent, s->threads, 0);
-        if (value < 1 || value > per_sm) return fail(TS_EINVAL, "blocks_per_sm must be in 1..%d", per_sm);
-        s->grid_persistent = sms * (int)value;
-        s->grid_plain = sms * (int)value;
+        if (value < 1 || value * s->threads > 2048) return fail(TS_EINVAL, "blocks_per_sm * threads must be in 1..2048");
+        s->blocks_per_sm = (int)value;
+    } else if (!strcmp(key, "threads")) {
+        if (value < 64 || value > 1024 || value % 32) return fail(TS_EINVAL, "threads must be a multiple of 32 in 64..1024");
+        s->threads = (int)value;
+        s->blocks_per_sm = std::min(s->blocks_per_sm, 2048 / s->threads);
+    } else if (!strcmp(key, "sort_period")) {
+        if (value < 0 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "sort_period must be >= 0");
+        s->sort_period = (uint32_t)value;
     } else return fail(TS_EINVAL, "unknown option '%s'", key);
     return TS_OK;
 }
@@ -464,15 +519,38 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
 static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
     if ((uint64_t)s->k + n >= 0x7FFFFFFFull) return fail(TS_EINVAL, "step counter would pass 2^31");
     cudaStream_t st = s->stream;
+    const uint32_t R = s->sort_period;
+    const uint32_t sorts = R ? (s->k + n) / R - s->k / R : 0;       // steps k with (k + 1) % R == 0
     if (s->mode == 1) {
-        uint32_t k0 = s->k;
-        void* args[] = {&s->ctx, &k0, &n, &d_digests};
-        CUDA_TRY(cudaLaunchCooperativeKernel((void*)k_persistent, dim3(s->grid_persistent), dim3(s->threads), args, 0, st));
+        // shared memory holds the move records of the first mr_j slots of every thread
+        const int per_sm_smem = (s->smem_limit - 1024) / s->blocks_per_sm - 1024;
+        uint32_t mr_j = (uint32_t)std::max(0, per_sm_smem / (16 * s->threads));
+        const uint32_t grid = (uint32_t)(s->sms * s->blocks_per_sm);
+        const uint32_t need_j = (s->L.cap + grid * s->threads - 1) / (grid * s->threads);
+        mr_j = std::min(mr_j, need_j);
+        const size_t smem = (size_t)mr_j * 16 * s->threads;
+        int per_sm = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent, s->threads, smem));
+        if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, s->threads);
+        CUDA_TRY(cudaMemsetAsync(s->ctx.barrier, 0, 4, st));
+        uint32_t k0 = s->k, cur = s->cur;
+        void* args[] = {&s->ctx, &k0, &n, &cur, (void*)&R, &mr_j, &d_digests};
+        CUDA_TRY(cudaLaunchCooperativeKernel((void*)k_persistent, dim3(grid), dim3(s->threads), args, smem, st));
+        if (sorts & 1) s->cur ^= 1;
     } else {
+        const int g = s->sms * 8, gs = std::min<int>(s->sms * 8, (int)kMaxCtas);
         for (uint32_t i = 0; i < n; i++) {
-            k_intent<<<s->grid_plain, s->threads, 0, st>>>(s->ctx, s->k + i);
-            k_commit<<<s->grid_plain, s->threads, 0, st>>>(s->ctx, s->k + i);
-            if (d_digests) k_digest<<<s->grid_plain, s->threads, 0, st>>>(s->ctx, d_digests + i);
+            const uint32_t k = s->k + i;
+            k_phase1<<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            k_phase2<<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            if (d_digests) k_digest<<<g, 256, 0, st>>>(s->ctx, s->cur, d_digests + i);
+            if (R && (k + 1) % R == 0) {
+                k_sort_rank<<<gs, 256, 0, st>>>(s->ctx, s->cur);
+                k_sort_partial<<<gs, 256, 0, st>>>(s->ctx);
+                k_sort_scan<<<gs, 256, 0, st>>>(s->ctx);
+                k_sort_scatter<<<gs, 256, 0, st>>>(s->ctx, s->cur);
+                s->cur ^= 1;
+            }
         }
         CUDA_TRY(cudaGetLastError());
     }
@@ -515,14 +593,23 @@ static int copy_out(ts_sim* s, void* dst, const void* src, size_t bytes) {
     return TS_OK;
 }
 
+static const char* describe(uint32_t err) {
+    if (err & ERR_CELL_CLASH) return "two vehicles scattered to one atlas cell";
+    if (err & ERR_SLOTS) return "slot overflow";
+    return "internal logic check failed";
+}
+
 extern "C" int ts_read_state(ts_sim* s, ts_state_out* o) {
     if (!s || !o) return fail(TS_EINVAL, "null argument");
     Layout& L = s->L;
     const size_t V = L.V;
-    const int g = std::max(1, std::min(1184, (int)((V + 255) / 256)));
-    k_gather_slots<<<g, 256, 0, s->stream>>>(s->ctx);
-    k_finish_state<<<g, 256, 0, s->stream>>>(s->ctx, at<uint32_t>(s, L.o_cell), at<uint32_t>(s, L.o_ridx));
-    CUDA_TRY(cudaGetLastError());
+    const bool arrays = o->status || o->edge || o->lane || o->cell || o->x || o->v || o->route_idx || o->insert_step || o->arrive_step;
+    if (arrays) {
+        const int g = std::max(1, std::min(1184, (int)((V + 255) / 256)));
+        k_gather_slots<<<1184, 256, 0, s->stream>>>(s->ctx, s->cur);
+        k_finish_state<<<g, 256, 0, s->stream>>>(s->ctx, at<uint32_t>(s, L.o_cell), at<uint32_t>(s, L.o_ridx));
+        CUDA_TRY(cudaGetLastError());
+    }
     int rc = 0;
     if ((rc = copy_out(s, o->status, s->ws + L.o_status, V))) return rc;
     if ((rc = copy_out(s, o->lane, s->ws + L.o_lane, V))) return rc;
@@ -536,10 +623,9 @@ extern "C" int ts_read_state(ts_sim* s, ts_state_out* o) {
     Dyn d;
     CUDA_TRY(cudaMemcpyAsync(&d, s->ws + L.dyn, sizeof d, cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
-    o->step = s->k; o->n_pending = d.n_pending; o->n_active = d.n_active; o->n_arrived = d.n_arrived;
+    o->step = s->k; o->n_pending = L.V - d.n_departed; o->n_active = d.n_departed - d.n_arrived; o->n_arrived = d.n_arrived;
     o->vehicle_updates = d.updates;
-    if (d.error) { s->sticky = d.error; return fail(TS_EINVARIANT, "device invariant violated (flags 0x%x): %s", d.error,
-                                                   (d.error & ERR_CELL_CLASH) ? "two vehicles scattered to one atlas cell" : "slot overflow"); }
+    if (d.error) { s->sticky = d.error; return fail(TS_EINVARIANT, "device invariant violated (flags 0x%x): %s", d.error, describe(d.error)); }
     return TS_OK;
 }
 

@@ -2,31 +2,34 @@
 // same code runs from the per-phase kernels and from the persistent cooperative kernel.
 // Rule set and notation: DESIGN.md section 2 (steps 2a-2f, 3, 4, 5); citations per block.
 //
-// The step is latency-bound, so each function is written as a short chain
-// of "trips" to L2: every load of a trip is issued before any of them is consumed.
-//   intent : slot state -> edge records + own-lane window -> next-edge / target-lane windows
-//            -> speed codes -> claims (fire and forget)
-//   commit : slot state + intent -> [crossers only: edge records -> claims] -> stores
+// Each function is written as a short chain of "trips" to L2: every load of a trip is issued
+// before any of them is consumed.
+//   phase 1 : slot state (A, B) -> edge records + own-lane window [+ C if it may leave the edge or
+//             evaluates a lane change] -> next-edge / target-lane windows [+ route entry] -> speed
+//             codes -> own state k+1, move record, claims (fire and forget)
+//   phase 2 : move record (shared memory) -> atlas update (fire and forget); crossing vehicles:
+//             claim words + crossing record + state in ONE trip -> stores
 #pragma once
 #include "ts_device.cuh"
 
 namespace ts {
 
-// ------------------------------------------------------------------ phase 1: intent
+// ------------------------------------------------------------------ phase 1: vehicles
 
-// DESIGN.md 2, step 2: one ACTIVE vehicle, reads state k and atlas M_k only.
-__device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint32_t k) {
+// DESIGN.md 2, steps 2a-2f for one slot.  Reads state k and atlas M_k only; returns the move
+// record that phase 2 applies.  `n_upd` counts ACTIVE vehicles advanced (the metric's unit).
+__device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, uint32_t slot, uint32_t k,
+                                                bool sample, uint32_t& n_upd) {
     const Params& p = c.p;
     // trip 1: slot state
-    const uint32_t meta = __ldcg(c.s_meta + slot);
-    if (!(meta >> 8)) return;
-    const uint32_t l = meta & 0xFFu;
-    const float x = __ldcg(c.s_x + slot), v = __ldcg(c.s_v + slot);
-    const uint32_t e = __ldcg(c.s_edge + slot), e2 = __ldcg(c.s_next + slot);
-    const uint32_t id = __ldcg(c.s_id + slot);
-    const float v0m = __ldcg(c.s_v0m + slot);
-    const uint32_t row = __ldcg(c.s_row + slot);
-    const float mand = __ldcg(c.s_mand + slot);
+    const uint4 sa = ldcg4(S.A + slot);
+    const uint4 sb = ldcg4(S.B + slot);
+    if (!(sa.w & ALIVE)) return make_uint4(0, 0, 0, MR_NONE);
+    n_upd++;
+    const float x = __uint_as_float(sa.x), v = __uint_as_float(sa.y);
+    const uint32_t row = sa.z, l = sa.w & 0xFu;
+    const uint32_t e = sb.x, e2 = sb.y, id = sb.z;
+    const float v0m = __uint_as_float(sb.w);
     const int ci = (int)floorf(x);
     const bool fast = p.H <= 128 && p.Hb <= 128;      // one 256-cell window covers a scan
 
@@ -52,16 +55,17 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     const int lim2 = min((int)E2.len - 1, Hp - 1);
     const uint32_t row2 = lane_row(E2, l2);
 
-    // 2d eligibility (readings R12, R14): known before any target-lane byte is read
+    // E5: the furthest this vehicle can get in one step; below the end of the edge it can neither
+    // arrive nor cross, above it lanes are not changed (readings R12, R14)
+    float reach = v + p.a_dt;
+    reach = reach * p.dt;
+    reach = x + reach;
+    const bool may_leave = !(reach < Cf);
     bool lc_eval = false;
     uint32_t lt = l, rowt = row;
-    if (p.lc_period != 0 && lanes >= 2) {
+    if (p.lc_period != 0 && lanes >= 2 && !may_leave) {
         const int lti = (int)l + ((k & 1u) ? -1 : +1);
-        float n = v + p.a_dt;
-        n = n * p.dt;
-        n = x + n;
-        if (lti >= 0 && lti < (int)lanes && x >= p.entry_zone_f && n < Cf &&
-            ((k >> 1) + id) % p.lc_period == 0) {
+        if (lti >= 0 && lti < (int)lanes && x >= p.entry_zone_f && ((k >> 1) + id) % p.lc_period == 0) {
             lc_eval = true;
             lt = (uint32_t)lti;
             rowt = lane_row(E, lt);
@@ -69,7 +73,9 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     }
     const int lo = max(0, ci - p.Hb);
 
-    // trip 3: next-edge window and target-lane windows, all in flight together
+    // trip 3: next-edge window, target-lane windows and the cold part of the slot state
+    uint4 sc = make_uint4(0, 0, 0, 0);
+    if (may_leave || lc_eval) sc = ldcg4(S.C + slot);
     int cL = -1, cL2 = -1, cLt = -1, cF = -1;
     if (fast) {
         Win w_next, w_ta, w_tb;
@@ -84,12 +90,13 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
         if (lc_eval) { cLt = scan_ahead(c.occ, rowt, ci, lim); cF = scan_behind(c.occ, rowt, lo, ci - 1); }
     }
 
-    // trip 4: speed codes of the vehicles found
-    uint32_t code_lead = 1, code_Lt = 1, code_F = 1;
+    // trip 4: speed codes of the vehicles found, and the route entry after the next edge
+    uint32_t code_lead = 1, code_Lt = 1, code_F = 1, e3 = NONE32;
     if (cL >= 0) code_lead = code_at(c.codes, row, cL);
     else if (cL2 >= 0) code_lead = code_at(c.codes, row2, cL2);
     if (cLt >= 0) code_Lt = code_at(c.codes, rowt, cLt);
     if (cF >= 0) code_F = code_at(c.codes, rowt, cF);
+    if (may_leave && !last && sc.x + 2 < sc.y) e3 = __ldg(c.route_edges + sc.x + 2);
 
     // 2b gaps (E3)
     const bool lead_on_edge = cL >= 0, has_lead = cL >= 0 || cL2 >= 0;
@@ -109,6 +116,7 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     const bool has_Lt = cLt >= 0;
     float s_Lt = 0.0f, at_c = 0.0f;
     if (lc_eval) {
+        const float mand = __uint_as_float(sc.w);
         const bool has_F = cF >= 0;
         const float vLt = speed_decode(code_Lt), vF = speed_decode(code_F);
         float s_lag = 0.0f;
@@ -162,172 +170,201 @@ __device__ __forceinline__ void vehicle_intent(const Ctx& c, uint32_t slot, uint
     if (dx > cap) { dx = cap; vt = 0.0f; }
     float xt = x + dx;
 
-    // 2f crossing intent and claims (one vehicle at a time; lowest id wins)
-    uint32_t act = ACT_STAY, nrow = accepted ? rowt : row;
+    // 2f + the part of step 4 that concerns nobody else: this vehicle's own state k+1
+    const uint32_t gc_from = (row << 7) + (uint32_t)ci;
+    const uint32_t k1 = k + 1;
     if (xt >= Cf) {
-        if (last) act = ACT_ARRIVE;
-        else if (may_cross) {
-            act = ACT_CROSS;
-            nrow = row2;
-            const unsigned long long w = claim_word(k, id);
-            atomicMin(c.lane_claim + E2.lane_base + l2, w);
-            if (ctrl == CTRL_PRIORITY) atomicMin(c.node_claim + E.to_node, w);
-        } else { xt = Cf - 0.0625f; vt = 0.0f; }
+        if (!may_leave) atomicOr(&c.dyn->error, ERR_LOGIC);
+        if (last) {                                    // ARRIVE: retires
+            stcg4(S.A + slot, make_uint4(__float_as_uint(Cf), __float_as_uint(vt), row, l));
+            c.o_status[id] = 2; c.o_arrive[id] = k1; c.o_x[id] = Cf; c.o_v[id] = vt;
+            c.o_edge[id] = e; c.o_lane[id] = (uint8_t)l; c.o_rpos[id] = sc.x;
+            atomicAdd(c.st_exited + e, 1u);
+            atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - sc.z));
+            atomicAdd(&c.dyn->n_arrived, 1u);
+            atomicAdd(&c.dyn->sum_arrive, (unsigned long long)k1);
+            return make_uint4(gc_from, NONE32, 0, MR_CLEAR);
+        }
+        if (may_cross) {                               // CROSS: claims (one vehicle at a
+            const unsigned long long w = claim_word(k, id);              // time; lowest id wins)
+            const uint32_t g2 = E2.lane_base + l2;
+            const uint32_t h = (ctrl == CTRL_PRIORITY) ? E.to_node : NONE32;
+            atomicMin(c.lane_claim + g2, w);
+            if (h != NONE32) atomicMin(c.node_claim + h, w);
+            stcg4(S.A + slot, make_uint4(__float_as_uint(xt), __float_as_uint(vt), row, l | ALIVE));
+            const float v0n = v0m * E2.vlim;
+            stcg4(c.cr + 2 * (size_t)slot, make_uint4(row2, (uint32_t)E2.len | (l2 << 16), __float_as_uint(v0n), __float_as_uint(Cf)));
+            stcg4(c.cr + 2 * (size_t)slot + 1, make_uint4(e3, (uint32_t)C, 0, 0));
+            return make_uint4(gc_from, g2, h, MR_CROSS);
+        }
+        xt = Cf - 0.0625f; vt = 0.0f;                   // held at a red line (R17)
     }
-    c.s_xt[slot] = xt;
-    c.s_vt[slot] = vt;
-    c.s_act[slot] = act | ((accepted ? lt : l) << 4);
-    c.s_nrow[slot] = nrow;
+    const uint32_t l_new = accepted ? lt : l, nrow = accepted ? rowt : row;
+    const uint32_t code = speed_code(vt);
+    stcg4(S.A + slot, make_uint4(__float_as_uint(xt), __float_as_uint(vt), nrow, l_new | ALIVE));
+    if (sample) {                                      // PAPER.md:437 one sample per minute
+        atomicAdd(c.st_samp_cnt + e, 1u);
+        atomicAdd(c.st_samp_code + e, (unsigned long long)(code - 1));
+    }
+    return make_uint4(gc_from, (nrow << 7) + (uint32_t)(int)floorf(xt), code, MR_MOVE);
 }
 
-// DESIGN.md 2, step 3: the head of one departure queue.
-__device__ __forceinline__ void departure_intent(const Ctx& c, uint32_t q, uint32_t k) {
-    uint32_t cand = NONE32;
-    const uint32_t head = __ldcg(c.queue_head + q);
-    if (head < __ldg(c.queue_off + q + 1) && __ldg(c.queue_dep + head) <= k) {
-        const EdgeRec E = load_edge(c.edges, __ldg(c.queue_edge + q));
-        const Win w = load_win(c.occ, E.row, 0);
+// DESIGN.md 2, step 3: the head of one departure queue.  A ready head takes
+// a slot (kept as the queue's reservation until it wins) and writes its not-yet-alive state right
+// away; phase 2 only flips it alive if it holds the lane claim.
+__device__ __forceinline__ void departure_phase1(const Ctx& c, const Slots& S, uint32_t q, uint32_t k) {
+    const uint4 qr = __ldg(c.queue_rec + q);           // { row, lane_base, end, edge }
+    const uint4 qs = ldcg4(c.queue_state + q);         // { head, dep step of the head, reserved slot, - }
+    uint4 cand = make_uint4(NONE32, 0, 0, 0);
+    if (qs.x < qr.z && qs.y <= k) {
+        const Win w = load_win(c.occ, qr.x, 0);
+        const uint4 d0 = __ldg(c.dep_rec + 2 * (size_t)qs.x), d1 = __ldg(c.dep_rec + 2 * (size_t)qs.x + 1);
+        uint32_t dep_next = NONE32;
+        if (qs.x + 1 < qr.z) dep_next = __ldg(&c.dep_rec[2 * (size_t)(qs.x + 1) + 1].z);
         if (first_occupied(w, 0, (int)c.p.insert_clear - 1) < 0) {
-            cand = __ldg(c.queue_veh + head);
-            atomicMin(c.lane_claim + E.lane_base, claim_word(k, cand));
+            uint32_t slot = qs.z;
+            if (slot == NONE32) {
+                slot = atomicAdd(&c.dyn->slot_alloc, 1u);
+                if (slot < c.cap_slots) c.queue_state[q].z = slot;
+            }
+            if (slot >= c.cap_slots) atomicOr(&c.dyn->error, ERR_SLOTS);
+            else {
+                stcg4(S.A + slot, make_uint4(0u, 0u, qr.x, 0u));                    // x = 0, v = 0, lane 0, not alive
+                stcg4(S.B + slot, make_uint4(qr.w, d1.y, d0.x, d0.y));
+                stcg4(S.C + slot, make_uint4(d0.w, d1.x, k + 1, d0.z));
+                atomicMin(c.lane_claim + qr.y, claim_word(k, d0.x));
+                cand = make_uint4(d0.x, slot, qs.x, dep_next);
+            }
         }
     }
     c.queue_cand[q] = cand;
 }
 
-__device__ __forceinline__ void phase_intent(const Ctx& c, uint32_t k, uint32_t tid, uint32_t nthreads) {
-    const uint32_t n_slots = __ldcg(&c.dyn->slot_alloc);   // nothing appends during this phase
-    if (tid == 0) {
-        c.dyn->n_slots = n_slots;
-        // every vehicle ACTIVE at step k is advanced once: the metric's unit of work
-        c.dyn->updates += __ldcg(&c.dyn->n_active);
+// ------------------------------------------------------------------ phase 2
+
+// Apply one move record; crossing vehicles resolve their claims first (step 4).
+__device__ __forceinline__ void vehicle_phase2(const Ctx& c, const Slots& S, uint32_t slot, uint32_t k,
+                                               bool sample, const uint4 mr) {
+    if (mr.w == MR_NONE) return;
+    if (mr.w == MR_MOVE) {
+        if (mr.x != mr.y) { atlas_vacate(c, mr.x); atlas_occupy(c, mr.y, mr.z); }
+        else c.codes[mr.y] = (uint8_t)mr.z;
+        return;
     }
-    for (uint32_t s = tid; s < n_slots; s += nthreads) vehicle_intent(c, s, k);
-    for (uint32_t q = tid; q < c.n_queues; q += nthreads) departure_intent(c, q, k);
-}
-
-// ------------------------------------------------------------------ phase 2: resolve + commit
-
-// Vacate (row_from, cell_from) and occupy (row_to, cell_to) with `code`.  Single buffer: no other
-// vehicle's new cell equals this vehicle's old cell (invariant I6), and bit updates commute, so
-// the integer atomics of different threads never conflict.  The bit that is already set when a
-// cell is occupied is the by-product that proves invariant I2 on the device.
-__device__ __forceinline__ void atlas_move(const Ctx& c, bool has_from, uint32_t row_from, int cell_from,
-                                           uint32_t row_to, int cell_to, uint32_t code) {
-    uint32_t* occ32 = reinterpret_cast<uint32_t*>(c.occ);
-    if (!has_from || row_from != row_to || cell_from != cell_to) {
-        if (has_from) atomicAnd(occ32 + ((size_t)row_from << 2) + (cell_from >> 5), ~(1u << (cell_from & 31)));
-        const uint32_t bit = 1u << (cell_to & 31);
-        const uint32_t old = atomicOr(occ32 + ((size_t)row_to << 2) + (cell_to >> 5), bit);
-        if (old & bit) atomicOr(&c.dyn->error, ERR_CELL_CLASH);
+    if (mr.w == MR_CLEAR) { atlas_vacate(c, mr.x); return; }
+    // MR_CROSS: one trip for everything
+    const uint4 sa = ldcg4(S.A + slot), sb = ldcg4(S.B + slot), sc = ldcg4(S.C + slot);
+    const uint4 c0 = ldcg4(c.cr + 2 * (size_t)slot), c1 = ldcg4(c.cr + 2 * (size_t)slot + 1);
+    const unsigned long long w = claim_word(k, sb.z);
+    const unsigned long long wl = __ldcg(c.lane_claim + mr.y);
+    const unsigned long long wn = (mr.z != NONE32) ? __ldcg(c.node_claim + mr.z) : w;
+    const uint32_t e = sb.x, e2 = sb.y, l = sa.w & 0xFu, k1 = k + 1;
+    float xn, vn;
+    uint32_t gc_to, e_new;
+    if (wl == w && wn == w) {                          // holds every claim it made: crosses
+        const uint32_t len2 = c0.y & 0xFFFFu, l2 = c0.y >> 16;
+        xn = __uint_as_float(sa.x) - __uint_as_float(c0.w);
+        xn = fminf(xn, (float)len2 - 0.0625f);
+        vn = fminf(__uint_as_float(sa.y), __uint_as_float(c0.z));       // R9
+        stcg4(S.A + slot, make_uint4(__float_as_uint(xn), __float_as_uint(vn), c0.x, l2 | ALIVE));
+        stcg4(S.B + slot, make_uint4(e2, c1.x, sb.z, sb.w));
+        stcg4(S.C + slot, make_uint4(sc.x + 1, sc.y, k1, sc.w));
+        atomicAdd(c.st_entered + e2, 1u);
+        atomicAdd(c.st_exited + e, 1u);
+        atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - sc.z));
+        gc_to = (c0.x << 7) + (uint32_t)(int)floorf(xn);
+        e_new = e2;
+    } else {                                           // lost a claim: held at the line (R15)
+        xn = __uint_as_float(c0.w) - 0.0625f; vn = 0.0f;
+        stcg4(S.A + slot, make_uint4(__float_as_uint(xn), 0u, sa.z, l | ALIVE));
+        gc_to = (sa.z << 7) + (c1.y - 1u);
+        e_new = e;
     }
-    c.codes[((size_t)row_to << 7) + cell_to] = (uint8_t)code;
-}
-
-__device__ __forceinline__ void vehicle_commit(const Ctx& c, uint32_t slot, uint32_t k, bool sample) {
-    // trip 1: slot state and intent
-    const uint32_t meta = __ldcg(c.s_meta + slot);
-    if (!(meta >> 8)) return;
-    const uint32_t l = meta & 0xFFu;
-    const uint32_t a = __ldcg(c.s_act + slot);
-    const uint32_t e = __ldcg(c.s_edge + slot);
-    const float x_old = __ldcg(c.s_x + slot);
-    float xn = __ldcg(c.s_xt + slot), vn = __ldcg(c.s_vt + slot);
-    const uint32_t row = __ldcg(c.s_row + slot);
-    uint32_t nrow = __ldcg(c.s_nrow + slot);
-    const uint32_t act = a & 15u;
-    uint32_t l_new = a >> 4, e_new = e;
-    const uint32_t k1 = k + 1;
-    const int c_old = (int)floorf(x_old);
-
-    if (act != ACT_STAY) {
-        const uint32_t id = __ldcg(c.s_id + slot);
-        const uint32_t e2 = __ldcg(c.s_next + slot);
-        const uint32_t enter = __ldcg(c.s_enter + slot);
-        const uint32_t rpos = __ldcg(c.s_rpos + slot);
-        const EdgeRec E = load_edge(c.edges, e);
-        if (act == ACT_CROSS) {
-            // trip 2: edge records and the route two edges ahead; trip 3: the claim words
-            const EdgeRec E2 = load_edge(c.edges, e2);
-            const uint32_t rend = __ldg(c.route_end + id);
-            const uint32_t e3 = (rpos + 2 < rend) ? __ldg(c.route_edges + rpos + 2) : NONE32;
-            const float v0m = __ldcg(c.s_v0m + slot);
-            const uint32_t lanes2 = edge_lanes(E2);
-            const uint32_t l2 = l < lanes2 - 1 ? l : lanes2 - 1;
-            const unsigned long long w = claim_word(k, id);
-            const unsigned long long wl = __ldcg(c.lane_claim + E2.lane_base + l2);
-            const unsigned long long wn = (edge_ctrl(E) == CTRL_PRIORITY) ? __ldcg(c.node_claim + E.to_node) : w;
-            const float Cf = (float)E.len;
-            if (wl == w && wn == w) {                  // holds every claim it made: crosses
-                xn = xn - Cf;
-                xn = fminf(xn, (float)E2.len - 0.0625f);
-                vn = fminf(vn, v0m * E2.vlim);         // R9
-                e_new = e2; l_new = l2;
-                c.s_rpos[slot] = rpos + 1;
-                c.s_next[slot] = e3;
-                c.s_edge[slot] = e2;
-                c.s_enter[slot] = k1;
-                atomicAdd(c.st_entered + e2, 1u);
-                atomicAdd(c.st_exited + e, 1u);
-                atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - enter));
-            } else {                                   // lost a claim: held at the line (R15)
-                xn = Cf - 0.0625f; vn = 0.0f; l_new = l; nrow = row;
-            }
-        } else {                                       // ACT_ARRIVE
-            atomicAnd(reinterpret_cast<uint32_t*>(c.occ) + ((size_t)row << 2) + (c_old >> 5), ~(1u << (c_old & 31)));
-            c.s_meta[slot] = l;                        // alive bit off
-            c.o_status[id] = 2; c.o_arrive[id] = k1; c.o_x[id] = (float)E.len; c.o_v[id] = vn;
-            c.o_edge[id] = e; c.o_lane[id] = (uint8_t)l; c.o_rpos[id] = rpos;
-            atomicAdd(c.st_exited + e, 1u);
-            atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - enter));
-            atomicSub(&c.dyn->n_active, 1u);
-            atomicAdd(&c.dyn->n_arrived, 1u);
-            atomicAdd(&c.dyn->sum_arrive, (unsigned long long)k1);
-            return;
-        }
-    }
-    c.s_x[slot] = xn;
-    c.s_v[slot] = vn;
-    if (l_new != l) c.s_meta[slot] = l_new | 0x100u;
-    if (nrow != row) c.s_row[slot] = nrow;
     const uint32_t code = speed_code(vn);
-    atlas_move(c, true, row, c_old, nrow, (int)floorf(xn), code);
-    if (sample) {                                      // PAPER.md:437 one sample per minute
+    if (mr.x != gc_to) { atlas_vacate(c, mr.x); atlas_occupy(c, gc_to, code); }
+    else c.codes[gc_to] = (uint8_t)code;
+    if (sample) {
         atomicAdd(c.st_samp_cnt + e_new, 1u);
         atomicAdd(c.st_samp_code + e_new, (unsigned long long)(code - 1));
     }
 }
 
 // DESIGN.md 2, step 4 (departures): the winning queue head becomes ACTIVE at x = 0, v = 0, lane 0.
-__device__ __forceinline__ void departure_commit(const Ctx& c, uint32_t q, uint32_t k, bool sample) {
-    const uint32_t id = __ldcg(c.queue_cand + q);
-    if (id == NONE32) return;
-    const uint32_t e = __ldg(c.queue_edge + q);
-    const EdgeRec E = load_edge(c.edges, e);
-    if (__ldcg(c.lane_claim + E.lane_base) != claim_word(k, id)) return;
-    const uint32_t slot = atomicAdd(&c.dyn->slot_alloc, 1u);
-    if (slot >= c.cap_slots) { atomicOr(&c.dyn->error, ERR_SLOTS); return; }
+__device__ __forceinline__ void departure_phase2(const Ctx& c, const Slots& S, uint32_t q, uint32_t k, bool sample) {
+    const uint4 cand = __ldcg(c.queue_cand + q);       // { id, slot, head, dep step of the next }
+    if (cand.x == NONE32) return;
+    const uint4 qr = __ldg(c.queue_rec + q);
+    if (__ldcg(c.lane_claim + qr.y) != claim_word(k, cand.x)) return;   // the slot stays dead
     const uint32_t k1 = k + 1;
-    const uint32_t rb = __ldg(c.route_begin + id);
-    c.s_x[slot] = 0.0f; c.s_v[slot] = 0.0f; c.s_edge[slot] = e; c.s_meta[slot] = 0x100u;
-    c.s_id[slot] = id; c.s_rpos[slot] = rb; c.s_enter[slot] = k1; c.s_row[slot] = E.row;
-    c.s_next[slot] = (rb + 1 < __ldg(c.route_end + id)) ? __ldg(c.route_edges + rb + 1) : NONE32;
-    c.s_v0m[slot] = __ldg(c.v0_mult + id); c.s_mand[slot] = __ldg(c.mand_dist + id);
-    c.o_status[id] = 1; c.o_insert[id] = k1;
-    c.queue_head[q] = __ldcg(c.queue_head + q) + 1;
-    atlas_move(c, false, 0, 0, E.row, 0, 1u);
-    atomicAdd(c.st_entered + e, 1u);
-    atomicSub(&c.dyn->n_pending, 1u);
-    atomicAdd(&c.dyn->n_active, 1u);
-    if (sample) atomicAdd(c.st_samp_cnt + e, 1u);  // speed code - 1 == 0 at rest
+    stcg4(S.A + cand.y, make_uint4(0u, 0u, qr.x, ALIVE));
+    c.o_status[cand.x] = 1; c.o_insert[cand.x] = k1;
+    c.queue_state[q] = make_uint4(cand.z + 1, cand.w, NONE32, 0);
+    atlas_occupy(c, qr.x << 7, 1u);
+    atomicAdd(c.st_entered + qr.w, 1u);
+    atomicAdd(&c.dyn->n_departed, 1u);
+    if (sample) atomicAdd(c.st_samp_cnt + qr.w, 1u);   // speed code - 1 == 0 at rest
 }
 
-__device__ __forceinline__ void phase_commit(const Ctx& c, uint32_t k, uint32_t tid, uint32_t nthreads) {
+// ------------------------------------------------------------------ phase drivers
+// `mr_s`: this CTA's move records in shared memory, [mr_j][T]; slots beyond that use c.mr_g.
+
+__device__ __forceinline__ uint32_t phase1(const Ctx& c, const Slots& S, uint32_t k, const Who& me, uint4* mr_s,
+                                           uint32_t mr_j, uint32_t& n_upd) {
     const uint32_t n_slots = __ldcg(&c.dyn->n_slots);
     const bool sample = c.p.sample_period && ((k + 1) % c.p.sample_period == 0);
-    if (tid == 0) { c.dyn->k = k + 1; if (sample) c.dyn->n_samples += 1; }
-    for (uint32_t s = tid; s < n_slots; s += nthreads) vehicle_commit(c, s, k, sample);
-    for (uint32_t q = tid; q < c.n_queues; q += nthreads) departure_commit(c, q, k, sample);
+    for (uint32_t j = 0;; j++) {
+        const uint32_t s = me.slot(j);
+        if (s >= n_slots) break;
+        const uint4 mr = vehicle_phase1(c, S, s, k, sample, n_upd);
+        if (j < mr_j) mr_s[j * me.T + me.t] = mr; else stcg4(c.mr_g + s, mr);
+    }
+    for (uint32_t q = me.gtid(); q < c.n_queues; q += me.gthreads()) departure_phase1(c, S, q, k);
+    return n_slots;
+}
+
+__device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k, const Who& me, const uint4* mr_s,
+                                       uint32_t mr_j, uint32_t n_slots) {
+    const bool sample = c.p.sample_period && ((k + 1) % c.p.sample_period == 0);
+    if (me.gtid() == 0) {
+        // every slot handed out in phase 1 takes part from the next step on
+        c.dyn->n_slots = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
+        c.dyn->k = k + 1;
+        if (sample) c.dyn->n_samples += 1;
+    }
+    for (uint32_t j = 0;; j++) {
+        const uint32_t s = me.slot(j);
+        if (s >= n_slots) break;
+        const uint4 mr = (j < mr_j) ? mr_s[j * me.T + me.t] : ldcg4(c.mr_g + s);
+        vehicle_phase2(c, S, s, k, sample, mr);
+    }
+    for (uint32_t q = me.gtid(); q < c.n_queues; q += me.gthreads()) departure_phase2(c, S, q, k, sample);
+}
+
+// order-independent digest of state k+1 (test instrument, not on the timed path).
+__device__ __forceinline__ void phase_digest(const Ctx& c, const Slots& S, unsigned long long* out, const Who& me) {
+    const uint32_t n_slots = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
+    unsigned long long sum = 0;
+    for (uint32_t j = 0;; j++) {
+        const uint32_t s = me.slot(j);
+        if (s >= n_slots) break;
+        const uint4 sa = ldcg4(S.A + s);
+        if (!(sa.w & ALIVE)) continue;
+        const uint4 sb = ldcg4(S.B + s);
+        unsigned long long g = mix64((unsigned long long)sb.z);
+        g = mix64(g ^ (((unsigned long long)sb.x << 8) | (sa.w & 0xFFu)));
+        g = mix64(g ^ (((unsigned long long)sa.x << 32) | (unsigned long long)sa.y));
+        sum += g;
+    }
+    if (me.gtid() == 0) {
+        const uint32_t dep = __ldcg(&c.dyn->n_departed), arr = __ldcg(&c.dyn->n_arrived);
+        unsigned long long g = mix64((unsigned long long)(c.V - dep));
+        g = mix64(g ^ (unsigned long long)(dep - arr));
+        g = mix64(g ^ (unsigned long long)arr);
+        g = mix64(g ^ __ldcg(&c.dyn->sum_arrive));
+        sum += g;
+    }
+    for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xFFFFFFFFu, sum, o);
+    if ((threadIdx.x & 31) == 0 && sum) atomicAdd(out, sum);
 }
 
 }  // namespace ts

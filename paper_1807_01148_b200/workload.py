@@ -362,3 +362,28 @@ def config5(n_vehicles=2_000_000, steps=28800, grid=256, core=8, workers=None):
     return _finish("cfg5_stress", rng, N, ef, et, np.full(E, 200), np.full(E, 2), np.full(E, 15.0),
                    np.full(N, CTRL_PRIORITY), (z, z, z), origins, dests, depart, steps,
                    np.ones(n_vehicles), None, xy, workers)
+
+
+def config3_dense(n_vehicles=1_000_000, steps=2400, workers=None):
+    """DIAGNOSTIC, not a sixth config: config 3's network with every departure
+    compressed into the first 60 s, so that ~1 M vehicles are active at once.  Separates kernel
+    efficiency from the per-step latency floor."""
+    return config3(n_vehicles=n_vehicles, steps=steps, workers=workers, depart_mean_s=30.0,
+                   depart_sd_s=15.0, name="cfg3_dense_diagnostic")
+
+
+_BY_NAME = {
+    "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg5": config5,
+    "cfg3_dense": config3_dense,
+    # quick functional checks, not reported workloads
+    "cfg3_small": lambda: config3(n_vehicles=50_000, steps=7200, grid=64, n_origin_nodes=512,
+                                  depart_mean_s=1200.0, depart_sd_s=400.0, name="cfg3_small"),
+    "cfg5_small": lambda: config5(n_vehicles=60_000, steps=7200, grid=48, core=4),
+}
+
+
+def by_name(name):
+    """Workload bundle by short name (bench.py --workload, tests/golden/make_golden.py)."""
+    if name not in _BY_NAME:
+        raise KeyError(f"unknown workload {name!r}; known: {sorted(_BY_NAME)}")
+    return _BY_NAME[name]()

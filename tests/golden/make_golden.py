@@ -1,0 +1,65 @@
+#!/usr/bin/env python
+"""Writes tests/golden/trace_<cfg>.json by running ONLY the oracle (oracle/) on the seeded
+workload of a BASELINE.json config, full length.
+
+    python tests/golden/make_golden.py cfg1 cfg2 cfg3 cfg5 [--stride 600]
+
+Stored per config (nothing here ever comes from the CUDA path):
+  sha256     checksum of the generated input bundle (detects generator drift between machines)
+  digests    the oracle's 64-bit state digest (SURVEY.md 8(d) "Parity") after steps
+             stride, 2*stride, ..., and after the last step -- the sampled outputs the
+             full-size GPU parity test compares against
+  active     number of ACTIVE vehicles at the same steps
+  counters   the oracle's work counters for the whole run: the cells a byte-scan method has to
+             look at per vehicle-update, used by bench.py for the algorithmic bytes per update
+  final      n_pending / n_active / n_arrived after the last step
+  seconds    single-thread wall time of the oracle run (context only)
+"""
+import argparse
+import json
+import os
+import sys
+import time
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+sys.path.insert(0, ROOT)
+
+from oracle import Oracle                                    # noqa: E402
+from paper_1807_01148_b200 import workload as W              # noqa: E402
+
+
+def run(name, stride):
+    bundle = W.by_name(name)
+    orc = Oracle(bundle)
+    steps = bundle["steps"]
+    marks, digests, active = [], [], []
+    t0 = time.perf_counter()
+    done = 0
+    while done < steps:
+        n = min(stride, steps - done)
+        d = orc.step(n, digests=True)
+        done += n
+        marks.append(done)
+        digests.append(f"{int(d[-1]):016x}")
+        active.append(int(orc.read_state()["n_active"]))
+    secs = time.perf_counter() - t0
+    st = orc.read_state()
+    out = dict(name=bundle["name"], sha256=W.bundle_sha256(bundle), steps=steps, stride=stride,
+               marks=marks, digests=digests, active=active, counters=orc.counters(),
+               final=dict(n_pending=int(st["n_pending"]), n_active=int(st["n_active"]),
+                          n_arrived=int(st["n_arrived"])),
+               seconds=round(secs, 1))
+    path = os.path.join(HERE, f"trace_{name}.json")
+    with open(path, "w") as f:
+        json.dump(out, f, indent=1)
+    print(name, "->", path, f"{secs:.0f} s", out["counters"]["updates"], "updates", flush=True)
+
+
+if __name__ == "__main__":
+    ap = argparse.ArgumentParser()
+    ap.add_argument("configs", nargs="+")
+    ap.add_argument("--stride", type=int, default=600)
+    a = ap.parse_args()
+    for c in a.configs:
+        run(c, a.stride)

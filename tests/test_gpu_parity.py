@@ -12,11 +12,13 @@ from test_oracle_pins import corridor
 pytestmark = pytest.mark.gpu
 
 
-def _compare(bundle, steps, mode, chunk=None):
+def _compare(bundle, steps, mode, chunk=None, **options):
     import paper_1807_01148_b200 as pkg
     from oracle import Oracle
     orc = Oracle(bundle)
     sim = pkg.Sim(bundle, "cuda:0", mode=mode)
+    for key, value in options.items():
+        sim.set_option(key, value)
     done = 0
     chunk = chunk or steps
     while done < steps:
@@ -51,6 +53,22 @@ def test_config1_full(cfg1, mode):
 def test_mixed_controls(mode):
     b = small_signal_grid()
     _compare(b, b["steps"], mode)
+
+
+@pytest.mark.parametrize("options", [
+    dict(sort_period=0),                       # never compacted: slots only grow
+    dict(sort_period=1),                       # compacted + re-sorted after every step
+    dict(sort_period=7, threads=128),          # several slots per thread, ragged tile tails
+    dict(sort_period=50, threads=512, blocks_per_sm=2),
+    dict(sort_period=3, threads=64),           # move records overflow shared memory into global
+])
+def test_results_do_not_depend_on_slot_order(options):
+    """A9/A10: compaction and the edge re-sort change where a vehicle's state lives, never what
+    it is; neither does the launch geometry."""
+    b = small_signal_grid()
+    _compare(b, b["steps"], 1, **options)
+    if options["sort_period"] in (0, 1):
+        _compare(b, 400, 0, sort_period=options["sort_period"])
 
 
 def test_corridors():
