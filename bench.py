@@ -157,6 +157,10 @@ def main():
     ap.add_argument("--sim-steps", type=int, default=0, help="override the config's simulation steps (diagnostics)")
     ap.add_argument("--start-step", type=int, default=0,
                     help="advance this many simulation steps untimed before the timed window (diagnostics)")
+    ap.add_argument("--threads", type=int, default=0, help="CTA size of the persistent kernel (tuning)")
+    ap.add_argument("--blocks-per-sm", type=int, default=0)
+    ap.add_argument("--sort-period", type=int, default=-1, help="steps between compaction + re-sort (tuning)")
+    ap.add_argument("--profile", action="store_true", help="clock the phases inside the persistent kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -187,6 +191,17 @@ def main():
     sim_steps = args.sim_steps or (bundle["steps"] - args.start_step)
     stream = torch.cuda.current_stream()
     sim = pkg.Sim(bundle, f"cuda:{local}", mode=args.mode)
+    tuning = {}
+    if args.threads:
+        tuning["threads"] = args.threads
+    if args.blocks_per_sm:
+        tuning["blocks_per_sm"] = args.blocks_per_sm
+    if args.sort_period >= 0:
+        tuning["sort_period"] = args.sort_period
+    if args.profile:
+        tuning["profile"] = 1
+    for key, val in tuning.items():
+        sim.set_option(key, val)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")   # > 126 MB L2
 
     def one_run():
@@ -216,6 +231,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     ms = [a.elapsed_time(b) for a, b, _ in evs]
     counts = sim.read_counts()
+    phase_ns = sim.read_profile() if args.profile else None
     updates = int(counts["vehicle_updates"]) - evs[-1][2]   # per timed window (reset zeroes the counter)
     total_ms = torch.tensor([sum(ms)], dtype=torch.float64, device=f"cuda:{local}")
     if dist is not None:
@@ -242,6 +258,8 @@ def main():
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         s2 = pkg.Sim(pinned, f"cuda:{local}", mode=args.mode)     # ts_query_workspace + ts_create: H2D
+        for key, val in tuning.items():
+            s2.set_option(key, val)
         s2.step(sim_steps)
         st = s2.read_state()                                       # D2H of the whole state
         e1.record(stream)
@@ -275,7 +293,7 @@ def main():
         "data": "synthetic",
         "config": {"workload": bundle["name"], "vehicles": V, "edges": bundle["n_edges"],
                    "sim_steps_per_bench_step": sim_steps, "vehicle_updates_per_bench_step": updates,
-                   "start_step": args.start_step,
+                   "start_step": args.start_step, "tuning": tuning, "phase_ns_per_sim_step": phase_ns,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "step_kernel": "persistent cooperative" if args.mode == 1 else "two launches per sim step",
                    "l2": "flushed between timed iterations (256 MiB fill) and inputs (routes+atlas) exceed L2"},

@@ -16,8 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libts.so")
 TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
-           "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_destroy", "ts_last_error",
-           "ts_version"]
+           "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile", "ts_destroy",
+           "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -87,11 +87,12 @@ def load():
         L.ts_read_state.argtypes = [C.c_void_p, C.c_void_p]
         L.ts_read_edge_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.ts_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
+        L.ts_read_profile.argtypes = [C.c_void_p, C.c_void_p]
         L.ts_destroy.argtypes = [C.c_void_p]
         L.ts_destroy.restype = None
         L.ts_last_error.restype = C.c_char_p
         L.ts_version.restype = C.c_char_p
-        for n in EXPORTS[:8]:
+        for n in EXPORTS[:9]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -185,6 +186,16 @@ class Sim:
         _check(load().ts_read_state(self._h, C.byref(o)))
         return dict(step=o.step, n_pending=o.n_pending, n_active=o.n_active, n_arrived=o.n_arrived,
                     vehicle_updates=o.vehicle_updates)
+
+    def read_profile(self):
+        """Option "profile": mean nanoseconds per simulation step in each phase (CTA 0's view)."""
+        a = np.zeros(8, np.uint64)
+        _check(load().ts_read_profile(self._h, a.ctypes.data))
+        n = max(1, int(a[6]))
+        names = ("phase1", "barrier1", "phase2", "barrier2", "sort", "digest")
+        out = {k: float(a[i]) / n for i, k in enumerate(names)}
+        out["steps"] = int(a[6])
+        return out
 
     def read_edge_stats(self, reset=False):
         E = self.E

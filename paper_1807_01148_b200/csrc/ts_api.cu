@@ -50,10 +50,10 @@ extern "C" const char* ts_version(void) {
 
 struct Layout {
     size_t total = 0;
-    uint32_t V = 0, E = 0, N = 0, Q = 0, cap = 0;
+    uint32_t V = 0, E = 0, N = 0, Q = 0, cap = 0, groups = 1;
     uint64_t R = 0, n_lanes = 0, atlas_chunks = 0;   // chunk = 128 cells of one lane row
     size_t edges, route_edges, route_begin, queue_rec, dep_rec, codes, occ, queue_state, queue_cand,
-        lane_claim, node_claim, dyn, barrier, slots, mr_g, cr, rank, hist, base, partial, o_status, o_lane,
+        lane_claim, node_claim, dyn, barrier, slots, mr_g, cr, rank, hist, base, audit, partial, o_status, o_lane,
         o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered, st_exited,
         st_exit_steps, st_samp_cnt, st_samp_code, digest;
     static constexpr uint32_t kDigestChunk = 8192;
@@ -69,13 +69,14 @@ struct Layout {
         queue_rec = take((size_t)Q * 16);
         dep_rec = take((size_t)V * 32);
         codes = take(atlas_chunks * 128);
-        occ = take((atlas_chunks + 2) * 16);          // two spare chunks: load_win never clamps
+        occ = take((atlas_chunks + 3) * 16);          // one spare chunk in front, two behind: load_win never clamps
         queue_state = take((size_t)Q * 16); queue_cand = take((size_t)Q * 16);
         lane_claim = take(n_lanes * 8); node_claim = take((size_t)N * 8);
         dyn = take(sizeof(Dyn)); barrier = take(256);
         slots = take((size_t)cap * 16 * 6);           // A, B, C in two ping-pong sets
         mr_g = take((size_t)cap * 16); cr = take((size_t)cap * 32);
-        rank = take((size_t)cap * 4); hist = take((size_t)E * 4); base = take((size_t)E * 4);
+        rank = take((size_t)cap * 4); hist = take((size_t)E * groups * 4); base = take((size_t)E * groups * 4);
+        audit = take(16);
         partial = take((size_t)kMaxCtas * 4);
         o_status = take(V); o_lane = take(V);
         o_edge = take((size_t)V * 4); o_x = take((size_t)V * 4); o_v = take((size_t)V * 4);
@@ -89,8 +90,11 @@ struct Layout {
 };
 
 // Sizes only (what ts_query_workspace may look at).
-static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
-    if (!net || !rt) return fail(TS_EINVAL, "null argument");
+static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_params* prm, Layout& L) {
+    if (!net || !rt || !prm) return fail(TS_EINVAL, "null argument");
+    // the re-sort groups vehicles by their place in the lane-change stagger when that is a mask
+    const uint32_t lcp = prm->lc_period;
+    L.groups = (lcp >= 2 && lcp <= 8 && !(lcp & (lcp - 1))) ? lcp : 1;
     if (net->n_edges == 0 || net->n_nodes == 0) return fail(TS_EINVAL, "empty network");
     if (rt->n_vehicles >= 0x7FFFFFF0u) return fail(TS_EINVAL, "too many vehicles");
     L.V = rt->n_vehicles; L.E = net->n_edges; L.N = net->n_nodes;
@@ -125,10 +129,10 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, Layout& L) {
 
 extern "C" int ts_query_workspace(const ts_network* net, const ts_routes* routes, const ts_departures* dep,
                                   const ts_params* params, size_t* bytes) {
-    (void)dep; (void)params;
+    (void)dep;
     if (!bytes) return fail(TS_EINVAL, "bytes is null");
     Layout L;
-    int rc = plan_sizes(net, routes, L);
+    int rc = plan_sizes(net, routes, params, L);
     if (rc) return rc;
     *bytes = L.total;
     return TS_OK;
@@ -145,10 +149,11 @@ struct ts_sim {
     uint32_t k = 0;           // steps enqueued so far
     uint32_t cur = 0;         // which slot set holds the state
     int mode = 1;             // 0: one launch per phase, 1: persistent cooperative kernel
-    int threads = 1024;       // persistent kernel CTA size
+    int threads = 512;        // persistent kernel CTA size (128 registers per thread: no spills)
     int blocks_per_sm = 1;
     int sms = 0;
     uint32_t sort_period = 64;   // steps between compaction + re-sort; 0 = never
+    uint32_t profile = 0;
     int smem_limit = 0;
     uint32_t sticky = 0;
 };
@@ -172,44 +177,83 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
     target += gridDim.x;
     __syncthreads();
     if (threadIdx.x == 0) {
-        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+        __threadfence();                                          // release, cumulative over the CTA
+        asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
         unsigned int v;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
+        do {                                                      // poll without a fence per probe
+            asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
         } while ((int)(v - target) < 0);
+        __threadfence();                                          // acquire
     }
     __syncthreads();
 }
 
 extern __shared__ uint4 dyn_smem[];
 
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// Phase clock of option "profile": thread 0 of CTA 0 adds the time since the last tick to bin b.
+struct PhaseClock {
+    unsigned long long* acc;   // shared memory, 8 bins; nullptr = off
+    unsigned long long last;
+    __device__ __forceinline__ void tick(int b) {
+        if (acc) { const unsigned long long t = global_ns(); acc[b] += t - last; last = t; }
+    }
+};
+
 // n steps in one launch; grid-wide barriers stand where the method has its two dependencies.
-__global__ void __launch_bounds__(1024, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
+// MAXT = most threads per SM it is launched with: sets the register budget (64 / 80 / 128).
+template <int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
                                                        uint32_t cur, uint32_t sort_period, uint32_t mr_j,
-                                                       unsigned long long* digests) {
+                                                       unsigned long long* digests, uint32_t profile) {
     __shared__ uint32_t red[33];
+    __shared__ uint32_t sh_n_slots[2];
+    __shared__ unsigned long long sh_prof[8];
     const Who me = who();
     unsigned int target = 0;
     uint32_t n_upd = 0;
+    PhaseClock clk;
+    clk.acc = (profile && me.gtid() == 0) ? sh_prof : nullptr;
+    if (clk.acc) { for (int b = 0; b < 8; b++) sh_prof[b] = 0; clk.last = global_ns(); }
+    if (me.t == 0) sh_n_slots[0] = __ldcg(&c.dyn->n_slots);
+    __syncthreads();
     for (uint32_t i = 0; i < n; i++) {
         const uint32_t k = k0 + i;
         const Slots& S = c.s[cur];
-        const uint32_t n_slots = phase1(c, S, k, me, dyn_smem, mr_j, n_upd);
+        const uint32_t n_slots = sh_n_slots[i & 1];
+        const bool sample = sample_step(c.p, k);
+        phase1(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd);
+        clk.tick(0);
         grid_barrier(c.barrier, target);
-        phase2(c, S, k, me, dyn_smem, mr_j, n_slots);
+        clk.tick(1);
+        // slots are handed out in phase 1 only: the count the next step works on is final now
+        if (me.t == 0) sh_n_slots[(i + 1) & 1] = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
+        phase2(c, S, k, me, dyn_smem, mr_j, n_slots, sample);
+        clk.tick(2);
         grid_barrier(c.barrier, target);
-        if (digests) phase_digest(c, S, digests + i, me);
+        clk.tick(3);
+        if (digests) { phase_digest(c, S, digests + i, me); clk.tick(5); }
         if (sort_period && (k + 1) % sort_period == 0) {      // A9 + A10, between two steps
-            const uint32_t ns = sort_rank(c, S, me);
+            const uint32_t ns = sort_rank(c, S, me, sh_n_slots[(i + 1) & 1]);
             grid_barrier(c.barrier, target);
             sort_partial(c, me, red);
             grid_barrier(c.barrier, target);
             sort_scan(c, me, red);
             grid_barrier(c.barrier, target);
             sort_scatter(c, S, c.s[cur ^ 1], me, ns);
+            if (me.t == 0) sh_n_slots[(i + 1) & 1] = __ldcg(&c.dyn->n_slots);
             grid_barrier(c.barrier, target);
             cur ^= 1;
+            clk.tick(4);
         }
+    }
+    if (clk.acc) {
+        for (int b = 0; b < 6; b++) c.dyn->prof[b] += sh_prof[b];
+        c.dyn->prof[6] += n;
     }
     n_upd = block_sum(n_upd, red);
     if (me.t == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
@@ -220,19 +264,29 @@ __global__ void __launch_bounds__(1024, 1) k_persistent(const __grid_constant__ 
 __global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
     __shared__ uint32_t red[33];
     uint32_t n_upd = 0;
-    const uint32_t n_slots = phase1(c, c.s[cur], k, who(), nullptr, 0, n_upd);
+    __shared__ uint32_t sh_n;
+    if (threadIdx.x == 0) sh_n = __ldcg(&c.dyn->n_slots);
+    __syncthreads();
+    const uint32_t n_slots = sh_n;
+    phase1(c, c.s[cur], k, who(), nullptr, 0, n_slots, sample_step(c.p, k), n_upd);
     if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n_slots;   // phase 2 overwrites dyn->n_slots
     n_upd = block_sum(n_upd, red);
     if (threadIdx.x == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
 }
 __global__ void __launch_bounds__(256) k_phase2(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
-    phase2(c, c.s[cur], k, who(), nullptr, 0, __ldcg(&c.dyn->pad));
+    __shared__ uint32_t sh_n;
+    if (threadIdx.x == 0) sh_n = __ldcg(&c.dyn->pad);
+    __syncthreads();
+    phase2(c, c.s[cur], k, who(), nullptr, 0, sh_n, sample_step(c.p, k));
 }
 __global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, uint32_t cur, unsigned long long* out) {
-    phase_digest(c, c.s[cur], out, who());
+    phase_digest(c, c.s[cur], out, who());   // test instrument: may read the slot count per thread
 }
 __global__ void __launch_bounds__(256) k_sort_rank(const __grid_constant__ Ctx c, uint32_t cur) {
-    const uint32_t n = sort_rank(c, c.s[cur], who());
+    __shared__ uint32_t sh_n;
+    if (threadIdx.x == 0) sh_n = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
+    __syncthreads();
+    const uint32_t n = sort_rank(c, c.s[cur], who(), sh_n);
     if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n;
 }
 __global__ void __launch_bounds__(256) k_sort_partial(const __grid_constant__ Ctx c) {
@@ -244,7 +298,10 @@ __global__ void __launch_bounds__(256) k_sort_scan(const __grid_constant__ Ctx c
     sort_scan(c, who(), red);
 }
 __global__ void __launch_bounds__(256) k_sort_scatter(const __grid_constant__ Ctx c, uint32_t cur) {
-    sort_scatter(c, c.s[cur], c.s[cur ^ 1], who(), __ldcg(&c.dyn->pad));
+    __shared__ uint32_t sh_n;
+    if (threadIdx.x == 0) sh_n = __ldcg(&c.dyn->pad);
+    __syncthreads();
+    sort_scatter(c, c.s[cur], c.s[cur ^ 1], who(), sh_n);
 }
 
 // State of step 0: every vehicle PENDING.
@@ -265,6 +322,31 @@ __global__ void k_init(const __grid_constant__ Ctx c) {
         memset(&d, 0, sizeof d);
         *c.dyn = d;
         *c.barrier = 0;
+    }
+}
+
+// Invariant I2 on the device, run when the state is read back: every ACTIVE vehicle's cell is
+// marked in the occupancy plane, and the plane holds exactly as many marked cells as there are
+// ACTIVE vehicles -- so no two vehicles share a cell and no mark was lost.
+__global__ void k_audit(const __grid_constant__ Ctx c, uint32_t cur, size_t n_words) {
+    const size_t tid = blockIdx.x * (size_t)blockDim.x + threadIdx.x, nthreads = gridDim.x * (size_t)blockDim.x;
+    const uint32_t* occ32 = reinterpret_cast<const uint32_t*>(c.occ);
+    unsigned long long marked = 0, missing = 0;
+    for (size_t i = tid; i < n_words; i += nthreads) marked += __popc(occ32[i]);
+    const uint32_t n_slots = min(c.dyn->slot_alloc, c.cap_slots);
+    for (size_t s = tid; s < n_slots; s += nthreads) {
+        const uint4 sa = c.s[cur].A[s];
+        if (!(sa.w & ALIVE)) continue;
+        const uint32_t gc = (sa.z << 7) + (uint32_t)(int)floorf(__uint_as_float(sa.x));
+        if (!((occ32[gc >> 5] >> (gc & 31)) & 1u)) missing++;
+    }
+    for (int o = 16; o; o >>= 1) {
+        marked += __shfl_xor_sync(0xFFFFFFFFu, marked, o);
+        missing += __shfl_xor_sync(0xFFFFFFFFu, missing, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (marked) atomicAdd(c.audit, marked);
+        if (missing) atomicAdd(c.audit + 1, missing);
     }
 }
 
@@ -351,12 +433,13 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     q.a_dt = p->a * p->dt;
     q.entry_zone_f = (float)p->entry_zone_cells;
     q.H = (int)p->lookahead_cells; q.Hb = (int)p->lookback_cells;
+    q.lc_pow2 = (p->lc_period && !(p->lc_period & (p->lc_period - 1))) ? 1u : 0u;
     q.lc_period = p->lc_period; q.insert_clear = p->insert_clear_cells; q.sample_period = p->sample_period_steps;
-    c.V = L.V; c.E = L.E; c.N = L.N; c.n_queues = L.Q; c.cap_slots = L.cap;
+    c.V = L.V; c.E = L.E; c.N = L.N; c.n_queues = L.Q; c.cap_slots = L.cap; c.sort_groups = L.groups;
     c.edges = at<EdgeRec>(s, L.edges); c.route_edges = at<uint32_t>(s, L.route_edges);
     c.route_begin = at<uint32_t>(s, L.route_begin);
     c.queue_rec = at<uint4>(s, L.queue_rec); c.dep_rec = at<uint4>(s, L.dep_rec);
-    c.codes = at<uint8_t>(s, L.codes); c.occ = at<uint4>(s, L.occ);
+    c.codes = at<uint8_t>(s, L.codes); c.occ = at<uint4>(s, L.occ) + 1;
     c.queue_state = at<uint4>(s, L.queue_state); c.queue_cand = at<uint4>(s, L.queue_cand);
     c.lane_claim = at<unsigned long long>(s, L.lane_claim); c.node_claim = at<unsigned long long>(s, L.node_claim);
     c.dyn = at<Dyn>(s, L.dyn); c.barrier = at<unsigned int>(s, L.barrier);
@@ -365,7 +448,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     for (int i = 0; i < 2; i++) { c.s[i].A = sl + (3 * i + 0) * cap; c.s[i].B = sl + (3 * i + 1) * cap; c.s[i].C = sl + (3 * i + 2) * cap; }
     c.mr_g = at<uint4>(s, L.mr_g); c.cr = at<uint4>(s, L.cr);
     c.rank = at<uint32_t>(s, L.rank); c.hist = at<uint32_t>(s, L.hist); c.base = at<uint32_t>(s, L.base);
-    c.partial = at<uint32_t>(s, L.partial);
+    c.partial = at<uint32_t>(s, L.partial); c.audit = at<unsigned long long>(s, L.audit);
     c.o_status = at<uint8_t>(s, L.o_status); c.o_lane = at<uint8_t>(s, L.o_lane);
     c.o_edge = at<uint32_t>(s, L.o_edge); c.o_x = at<float>(s, L.o_x); c.o_v = at<float>(s, L.o_v);
     c.o_rpos = at<uint32_t>(s, L.o_rpos); c.o_insert = at<uint32_t>(s, L.o_insert); c.o_arrive = at<uint32_t>(s, L.o_arrive);
@@ -378,10 +461,10 @@ extern "C" int ts_reset(ts_sim* s) {
     if (!s) return fail(TS_EINVAL, "null sim");
     Layout& L = s->L;
     cudaStream_t st = s->stream;
-    CUDA_TRY(cudaMemsetAsync(s->ws + L.occ, 0, (L.atlas_chunks + 2) * 16, st));   // codes need no clearing
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.occ, 0, (L.atlas_chunks + 3) * 16, st));   // codes need no clearing
     CUDA_TRY(cudaMemsetAsync(s->ws + L.lane_claim, 0xFF, L.n_lanes * 8, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.node_claim, 0xFF, (size_t)L.N * 8, st));
-    CUDA_TRY(cudaMemsetAsync(s->ws + L.hist, 0, (size_t)L.E * 4, st));
+    CUDA_TRY(cudaMemsetAsync(s->ws + L.hist, 0, (size_t)L.E * L.groups * 4, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, st));
     k_init<<<std::max(1u, std::min(1184u, (L.V + 255) / 256)), 256, 0, st>>>(s->ctx);
     CUDA_TRY(cudaGetLastError());
@@ -397,8 +480,9 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(TS_ECUDA, "no CUDA device: this library has no CPU fallback");
     Layout L;
-    int rc = plan_sizes(net, rt, L);
+    int rc = plan_sizes(net, rt, p, L);
     if (rc) return rc;
+    if ((uint64_t)L.groups * L.E >= 0xFFFFFFF0ull) L.groups = 1;
     if ((rc = validate(net, rt, dep, p))) return rc;
     if (!dev->workspace || ((uintptr_t)dev->workspace & 255)) return fail(TS_EINVAL, "workspace must be a 256-byte aligned device pointer");
     if (dev->bytes < L.total) return fail(TS_ENOMEM, "workspace too small: %zu < %zu bytes", dev->bytes, L.total);
@@ -484,7 +568,9 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     cudaGetDevice(&dev_id);
     cudaDeviceGetAttribute(&s->sms, cudaDevAttrMultiProcessorCount, dev_id);
     cudaDeviceGetAttribute(&s->smem_limit, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_id);
-    if (cudaFuncSetAttribute(k_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess) {
+    if (cudaFuncSetAttribute(k_persistent<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_persistent<768>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_persistent<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess) {
         delete s;
         return fail(TS_ECUDA, "cannot raise the dynamic shared memory limit of the step kernel");
     }
@@ -507,6 +593,8 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
         if (value < 64 || value > 1024 || value % 32) return fail(TS_EINVAL, "threads must be a multiple of 32 in 64..1024");
         s->threads = (int)value;
         s->blocks_per_sm = std::min(s->blocks_per_sm, 2048 / s->threads);
+    } else if (!strcmp(key, "profile")) {
+        s->profile = value ? 1u : 0u;
     } else if (!strcmp(key, "sort_period")) {
         if (value < 0 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "sort_period must be >= 0");
         s->sort_period = (uint32_t)value;
@@ -529,13 +617,15 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
         const uint32_t need_j = (s->L.cap + grid * s->threads - 1) / (grid * s->threads);
         mr_j = std::min(mr_j, need_j);
         const size_t smem = (size_t)mr_j * 16 * s->threads;
+        const int per_sm_threads = s->threads * s->blocks_per_sm;
+        void* kern = per_sm_threads <= 512 ? (void*)k_persistent<512> : per_sm_threads <= 768 ? (void*)k_persistent<768> : (void*)k_persistent<1024>;
         int per_sm = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent, s->threads, smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, s->threads, smem));
         if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, s->threads);
         CUDA_TRY(cudaMemsetAsync(s->ctx.barrier, 0, 4, st));
         uint32_t k0 = s->k, cur = s->cur;
-        void* args[] = {&s->ctx, &k0, &n, &cur, (void*)&R, &mr_j, &d_digests};
-        CUDA_TRY(cudaLaunchCooperativeKernel((void*)k_persistent, dim3(grid), dim3(s->threads), args, smem, st));
+        void* args[] = {&s->ctx, &k0, &n, &cur, (void*)&R, &mr_j, &d_digests, &s->profile};
+        CUDA_TRY(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(s->threads), args, smem, st));
         if (sorts & 1) s->cur ^= 1;
     } else {
         const int g = s->sms * 8, gs = std::min<int>(s->sms * 8, (int)kMaxCtas);
@@ -594,7 +684,7 @@ static int copy_out(ts_sim* s, void* dst, const void* src, size_t bytes) {
 }
 
 static const char* describe(uint32_t err) {
-    if (err & ERR_CELL_CLASH) return "two vehicles scattered to one atlas cell";
+    if (err & ERR_CELL_CLASH) return "atlas audit failed: two vehicles in one lane cell, or a vehicle whose cell is not marked";
     if (err & ERR_SLOTS) return "slot overflow";
     return "internal logic check failed";
 }
@@ -620,12 +710,27 @@ extern "C" int ts_read_state(ts_sim* s, ts_state_out* o) {
     if ((rc = copy_out(s, o->route_idx, s->ws + L.o_ridx, V * 4))) return rc;
     if ((rc = copy_out(s, o->insert_step, s->ws + L.o_insert, V * 4))) return rc;
     if ((rc = copy_out(s, o->arrive_step, s->ws + L.o_arrive, V * 4))) return rc;
+    unsigned long long audit[2];
+    CUDA_TRY(cudaMemsetAsync(s->ctx.audit, 0, 16, s->stream));
+    k_audit<<<1184, 256, 0, s->stream>>>(s->ctx, s->cur, (size_t)L.atlas_chunks * 4);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(audit, s->ctx.audit, 16, cudaMemcpyDeviceToHost, s->stream));
     Dyn d;
     CUDA_TRY(cudaMemcpyAsync(&d, s->ws + L.dyn, sizeof d, cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
+    if (audit[1] || audit[0] != (unsigned long long)(d.n_departed - d.n_arrived)) d.error |= ERR_CELL_CLASH;
     o->step = s->k; o->n_pending = L.V - d.n_departed; o->n_active = d.n_departed - d.n_arrived; o->n_arrived = d.n_arrived;
     o->vehicle_updates = d.updates;
     if (d.error) { s->sticky = d.error; return fail(TS_EINVARIANT, "device invariant violated (flags 0x%x): %s", d.error, describe(d.error)); }
+    return TS_OK;
+}
+
+extern "C" int ts_read_profile(ts_sim* s, uint64_t out[8]) {
+    if (!s || !out) return fail(TS_EINVAL, "null argument");
+    Dyn d;
+    CUDA_TRY(cudaMemcpyAsync(&d, s->ws + s->L.dyn, sizeof d, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    for (int b = 0; b < 8; b++) out[b] = d.prof[b];
     return TS_OK;
 }
 

@@ -63,6 +63,9 @@ struct Dyn {
     uint32_t k;            // step counter
     uint32_t pad;
     unsigned long long sum_arrive, updates;
+    // option "profile": nanoseconds CTA 0 spent in { phase 1, barrier 1, phase 2, barrier 2,
+    // compaction + re-sort, digest }, and the number of steps they cover
+    unsigned long long prof[8];
 };
 
 struct Params {
@@ -73,7 +76,12 @@ struct Params {
     float entry_zone_f;
     int H, Hb;
     uint32_t lc_period, insert_clear, sample_period;
+    uint32_t lc_pow2;      // lc_period is a power of two: the stagger test is a mask
 };
+// a sample is taken with the state after every sample_period-th step.
+__device__ __forceinline__ bool sample_step(const Params& p, uint32_t k) {
+    return p.sample_period && ((k + 1) % p.sample_period == 0);
+}
 
 // Slot-ordered vehicle state: three 16-byte vectors per slot (two ping-pong sets, swapped by
 // the re-sort).
@@ -90,6 +98,7 @@ struct Slots {
 struct Ctx {
     Params p;
     uint32_t V, E, N, n_queues, cap_slots;
+    uint32_t sort_groups;               // re-sort key = (id & (sort_groups - 1)) * E + edge
     // static network / demand
     const EdgeRec* edges;               // [E]
     const uint32_t* route_edges;        // [R]
@@ -110,8 +119,9 @@ struct Ctx {
     uint4* cr;                          // [2 cap] crossing records
     // compaction + re-sort scratch
     uint32_t* rank;                     // [cap]
-    uint32_t* hist;                     // [E]
-    uint32_t* base;                     // [E]
+    uint32_t* hist;                     // [sort_groups * E]
+    uint32_t* base;                     // [sort_groups * E]
+    unsigned long long* audit;          // [2] occupied cells counted / vehicles whose cell is not marked
     uint32_t* partial;                  // [kMaxCtas]
     // id-ordered results
     uint8_t* o_status; uint8_t* o_lane; uint32_t* o_edge; float* o_x; float* o_v;
@@ -127,7 +137,12 @@ constexpr uint32_t kMaxCtas = 2048;
 // robin, so that consecutive (edge-sorted) slots sit in consecutive lanes of one warp.
 struct Who {
     uint32_t t, T, cta, n_cta;
-    __device__ __forceinline__ uint32_t slot(uint32_t j) const { return (j * n_cta + cta) * T + t; }
+    // Slots (and departure queues) are dealt out in tiles of 32 -- one warp -- round robin over the
+    // CTAs first and the warps of a CTA second: a few thousand vehicles spread over all SMs (the
+    // step is bound by latency then), and consecutive edge-sorted slots share a warp.
+    __device__ __forceinline__ uint32_t slot(uint32_t j) const {
+        return ((j * (T >> 5) + (t >> 5)) * n_cta + cta) * 32u + (t & 31u);
+    }
     __device__ __forceinline__ uint32_t gtid() const { return cta * T + t; }
     __device__ __forceinline__ uint32_t gthreads() const { return n_cta * T; }
 };
@@ -193,68 +208,70 @@ __device__ __forceinline__ unsigned long long claim_word(uint32_t k, uint32_t id
 // ---- occupancy windows: 256 cells = two 16-byte chunks of one lane row, loaded together ----
 struct Win {
     uint4 a, b;   // chunk ch and chunk ch+1
-    int base;     // cell index of bit 0 of a
 };
-// `row` = first chunk of the lane row, `ch` = first chunk wanted.  Both loads are unconditional:
-// chunk ch+1 may belong to the next row (the plane ends with two spare chunks), callers mask by
-// the last cell of the edge, so no clamping -- and no dependence on the edge record -- is needed.
+// `row` = first chunk of the lane row, `ch` = first chunk wanted (-1 is legal: the plane has one
+// spare chunk in front and two behind).  Both loads are unconditional: a neighbouring chunk may
+// belong to another lane's row; callers bound the RESULT by the cells they may look at, so no
+// clamping -- and no dependence on the edge record -- is needed before the loads are issued.
 __device__ __forceinline__ Win load_win(const uint4* occ, uint32_t row, int ch) {
     Win w;
-    w.base = ch << 7;
-    w.a = __ldcg(occ + row + ch);
-    w.b = __ldcg(occ + row + ch + 1);
+    const uint4* p = occ + (ptrdiff_t)row + ch;
+    w.a = __ldcg(p);
+    w.b = __ldcg(p + 1);
     return w;
 }
-__device__ __forceinline__ uint32_t win_word(const Win& w, int i) {
-    switch (i) {
-        case 0: return w.a.x; case 1: return w.a.y; case 2: return w.a.z; case 3: return w.a.w;
-        case 4: return w.b.x; case 5: return w.b.y; case 6: return w.b.z; default: return w.b.w;
-    }
+// 160 bits of the window starting at bit f (0 <= f < 128): a[0] bit 0 is window bit f.  A two-
+// stage word barrel plus funnel shifts: no dynamic register indexing, no per-word masks.
+struct Bits160 { uint32_t a0, a1, a2, a3, a4; };
+__device__ __forceinline__ Bits160 extract160(const Win& w, int f) {
+    uint32_t w0 = w.a.x, w1 = w.a.y, w2 = w.a.z, w3 = w.a.w, w4 = w.b.x, w5 = w.b.y, w6 = w.b.z, w7 = w.b.w;
+    if (f & 64) { w0 = w2; w1 = w3; w2 = w4; w3 = w5; w4 = w6; w5 = w7; }
+    if (f & 32) { w0 = w1; w1 = w2; w2 = w3; w3 = w4; w4 = w5; }
+    const uint32_t sh = (uint32_t)f & 31u;
+    Bits160 r;
+    r.a0 = __funnelshift_r(w0, w1, sh);
+    r.a1 = __funnelshift_r(w1, w2, sh);
+    r.a2 = __funnelshift_r(w2, w3, sh);
+    r.a3 = __funnelshift_r(w3, w4, sh);
+    r.a4 = w4 >> sh;
+    return r;
 }
-// "we check the following bytes in memory": first occupied cell in [from, to]
-// (inclusive, cells of the window), or -1.
-__device__ __forceinline__ int first_occupied(const Win& w, int from, int to) {
-    const int f = from - w.base, t = to - w.base;      // bit indices in [0, 256)
-    if (f > t) return -1;
-#pragma unroll
-    for (int i = 0; i < 8; i++) {
-        const int lo = i << 5;
-        uint32_t m = win_word(w, i);
-        if (f > lo) m &= (f - lo >= 32) ? 0u : (0xFFFFFFFFu << (f - lo));
-        if (t < lo + 31) m &= (t < lo) ? 0u : (0xFFFFFFFFu >> (lo + 31 - t));
-        if (m) return w.base + lo + __ffs((int)m) - 1;
-    }
-    return -1;
+// "we check the following bytes in memory": the first occupied cell among the n
+// cells (n <= 129) that start at cell `from`; `w` must hold the chunk of `from` and the one after.
+// Returns the cell index or -1.  Bits beyond the n-th need no masking: if the first set bit lies
+// beyond them, none lies within.
+__device__ __forceinline__ int first_occupied(const Win& w, int from, int n) {
+    const Bits160 b = extract160(w, from & 127);
+    const unsigned long long lo = ((unsigned long long)b.a1 << 32) | b.a0, hi = ((unsigned long long)b.a3 << 32) | b.a2;
+    int pos = 128 + ((b.a4 & 1u) ? 0 : 64);
+    if (hi) pos = 63 + __ffsll((long long)hi);
+    if (lo) pos = __ffsll((long long)lo) - 1;
+    return pos < n ? from + pos : -1;
 }
-// Last occupied cell in [from, to] (the lag vehicle), or -1.
-__device__ __forceinline__ int last_occupied(const Win& w, int from, int to) {
-    const int f = from - w.base, t = to - w.base;
-    if (f > t) return -1;
-#pragma unroll
-    for (int i = 7; i >= 0; i--) {
-        const int lo = i << 5;
-        uint32_t m = win_word(w, i);
-        if (f > lo) m &= (f - lo >= 32) ? 0u : (0xFFFFFFFFu << (f - lo));
-        if (t < lo + 31) m &= (t < lo) ? 0u : (0xFFFFFFFFu >> (lo + 31 - t));
-        if (m) return w.base + lo + 31 - __clz((int)m);
-    }
-    return -1;
+// The last occupied cell among the n cells (n <= 128) that END at cell `last` (the lag vehicle,
+// PAPER.md:400); `w` must hold the chunk before the chunk of `last`, and the chunk of `last`.
+__device__ __forceinline__ int last_occupied(const Win& w, int last, int n) {
+    // window bit of `last` is 128 + (last & 127); take the 160 bits that start 128 below it, so
+    // that `last` is bit 128 and the cells below it are bits 127 .. 1
+    const Bits160 b = extract160(w, last & 127);
+    const unsigned long long lo = (((unsigned long long)b.a1 << 32) | b.a0) & ~1ull, hi = ((unsigned long long)b.a3 << 32) | b.a2;
+    int back = 192;                                   // distance behind `last`
+    if (lo) back = 65 + __clzll((long long)lo);       // bit p of lo is 128 - p cells behind
+    if (hi) back = 1 + __clzll((long long)hi);        // bit p of hi is  64 - p cells behind
+    if (b.a4 & 1u) back = 0;
+    return back < n ? last - back : -1;
 }
-// General ranges (lookahead > 128 cells): window after window.
+// General ranges (lookahead > 128 cells): 128 cells at a time.
 __device__ __forceinline__ int scan_ahead(const uint4* occ, uint32_t row, int from, int to) {
-    if (from > to) return -1;
-    for (int ch = from >> 7; ch <= (to >> 7); ch += 2) {
-        const Win w = load_win(occ, row, ch);
-        const int c = first_occupied(w, max(from, w.base), min(to, w.base + 255));
+    for (; from <= to; from += 128) {
+        const int c = first_occupied(load_win(occ, row, from >> 7), from, min(128, to - from + 1));
         if (c >= 0) return c;
     }
     return -1;
 }
 __device__ __forceinline__ int scan_behind(const uint4* occ, uint32_t row, int from, int to) {
-    if (from > to) return -1;
-    for (int ch = to >> 7; ch >= (from >> 7); ch -= 2) {
-        const Win w = load_win(occ, row, max(ch - 1, 0));
-        const int c = last_occupied(w, max(from, w.base), min(to, w.base + 255));
+    for (; to >= from; to -= 128) {
+        const int c = last_occupied(load_win(occ, row, (to >> 7) - 1), to, min(128, to - from + 1));
         if (c >= 0) return c;
     }
     return -1;
@@ -265,15 +282,27 @@ __device__ __forceinline__ uint32_t code_at(const uint8_t* codes, uint32_t row, 
 
 // Atlas cell address: the atlas holds < 2^32 cells (checked at ts_create), so (row, cell) packs
 // into one 32-bit global cell index gc = row * 128 + cell.
+//
+// Moving a vehicle vacates its old cell and occupies its new one with fire-and-forget integer
+// reductions (no return value is waited for).  Single buffer: no other vehicle's new cell equals
+// this vehicle's old cell (invariant I6) and bit updates commute, so threads never conflict.
+// Invariant I2 (no two vehicles in one lane cell) is audited when the state is read back
+// (k_audit): every ACTIVE vehicle's cell is marked and the number of marked cells equals the
+// number of ACTIVE vehicles.
+__device__ __forceinline__ void atlas_move(const Ctx& c, uint32_t gc_from, uint32_t gc_to, uint32_t code) {
+    uint32_t* occ32 = reinterpret_cast<uint32_t*>(c.occ);
+    if (gc_from != gc_to) {
+        const uint32_t bf = 1u << (gc_from & 31), bt = 1u << (gc_to & 31);
+        if ((gc_from >> 5) == (gc_to >> 5)) atomicXor(occ32 + (gc_to >> 5), bf | bt);
+        else { atomicAnd(occ32 + (gc_from >> 5), ~bf); atomicOr(occ32 + (gc_to >> 5), bt); }
+    }
+    c.codes[gc_to] = (uint8_t)code;
+}
 __device__ __forceinline__ void atlas_vacate(const Ctx& c, uint32_t gc) {
     atomicAnd(reinterpret_cast<uint32_t*>(c.occ) + (gc >> 5), ~(1u << (gc & 31)));
 }
-// The bit that is already set when a cell is occupied is the by-product that proves invariant
-// I2 (no two vehicles in one lane cell) on the device.
 __device__ __forceinline__ void atlas_occupy(const Ctx& c, uint32_t gc, uint32_t code) {
-    const uint32_t bit = 1u << (gc & 31);
-    const uint32_t old = atomicOr(reinterpret_cast<uint32_t*>(c.occ) + (gc >> 5), bit);
-    if (old & bit) atomicOr(&c.dyn->error, ERR_CELL_CLASH);
+    atomicOr(reinterpret_cast<uint32_t*>(c.occ) + (gc >> 5), 1u << (gc & 31));
     c.codes[gc] = (uint8_t)code;
 }
 

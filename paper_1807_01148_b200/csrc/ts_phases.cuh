@@ -50,6 +50,7 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     const uint32_t ctrl = edge_ctrl(E);
     const bool may_cross = last || ctrl != CTRL_SIGNAL || signal_green(E, k);
     const int lim = min(C - 1, ci + p.H);
+    const int n_own = lim - ci;                        // cells c+1 .. min(C-1, c+H)
     const int Hp = p.H - (C - 1 - ci);
     const bool want_next = !last && may_cross && Hp > 0;
     const int lim2 = min((int)E2.len - 1, Hp - 1);
@@ -65,7 +66,9 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     uint32_t lt = l, rowt = row;
     if (p.lc_period != 0 && lanes >= 2 && !may_leave) {
         const int lti = (int)l + ((k & 1u) ? -1 : +1);
-        if (lti >= 0 && lti < (int)lanes && x >= p.entry_zone_f && ((k >> 1) + id) % p.lc_period == 0) {
+        const uint32_t turn = (k >> 1) + id;           // staggered: every lc_period-th pair of steps
+        const bool my_turn = p.lc_pow2 ? (turn & (p.lc_period - 1u)) == 0u : turn % p.lc_period == 0u;
+        if (lti >= 0 && lti < (int)lanes && x >= p.entry_zone_f && my_turn) {
             lc_eval = true;
             lt = (uint32_t)lti;
             rowt = lane_row(E, lt);
@@ -80,10 +83,10 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     if (fast) {
         Win w_next, w_ta, w_tb;
         if (want_next) w_next = load_win(c.occ, row2, 0);
-        if (lc_eval) { w_ta = load_win(c.occ, rowt, ci >> 7); w_tb = load_win(c.occ, rowt, lo >> 7); }
-        cL = first_occupied(w_own, ci + 1, lim);                       // 2b
-        if (cL < 0 && want_next) cL2 = first_occupied(w_next, 0, lim2);
-        if (lc_eval) { cLt = first_occupied(w_ta, ci, lim); cF = last_occupied(w_tb, lo, ci - 1); }
+        if (lc_eval) { w_ta = load_win(c.occ, rowt, ci >> 7); w_tb = load_win(c.occ, rowt, ((ci - 1) >> 7) - 1); }
+        cL = first_occupied(w_own, ci + 1, n_own);                     // 2b
+        if (cL < 0 && want_next) cL2 = first_occupied(w_next, 0, lim2 + 1);
+        if (lc_eval) { cLt = first_occupied(w_ta, ci, lim - ci + 1); cF = last_occupied(w_tb, ci - 1, ci - lo); }
     } else {
         cL = scan_ahead(c.occ, row, ci + 1, lim);
         if (cL < 0 && want_next) cL2 = scan_ahead(c.occ, row2, 0, lim2);
@@ -221,7 +224,7 @@ __device__ __forceinline__ void departure_phase1(const Ctx& c, const Slots& S, u
         const uint4 d0 = __ldg(c.dep_rec + 2 * (size_t)qs.x), d1 = __ldg(c.dep_rec + 2 * (size_t)qs.x + 1);
         uint32_t dep_next = NONE32;
         if (qs.x + 1 < qr.z) dep_next = __ldg(&c.dep_rec[2 * (size_t)(qs.x + 1) + 1].z);
-        if (first_occupied(w, 0, (int)c.p.insert_clear - 1) < 0) {
+        if (first_occupied(w, 0, (int)c.p.insert_clear) < 0) {
             uint32_t slot = qs.z;
             if (slot == NONE32) {
                 slot = atomicAdd(&c.dyn->slot_alloc, 1u);
@@ -247,8 +250,7 @@ __device__ __forceinline__ void vehicle_phase2(const Ctx& c, const Slots& S, uin
                                                bool sample, const uint4 mr) {
     if (mr.w == MR_NONE) return;
     if (mr.w == MR_MOVE) {
-        if (mr.x != mr.y) { atlas_vacate(c, mr.x); atlas_occupy(c, mr.y, mr.z); }
-        else c.codes[mr.y] = (uint8_t)mr.z;
+        atlas_move(c, mr.x, mr.y, mr.z);
         return;
     }
     if (mr.w == MR_CLEAR) { atlas_vacate(c, mr.x); return; }
@@ -281,8 +283,7 @@ __device__ __forceinline__ void vehicle_phase2(const Ctx& c, const Slots& S, uin
         e_new = e;
     }
     const uint32_t code = speed_code(vn);
-    if (mr.x != gc_to) { atlas_vacate(c, mr.x); atlas_occupy(c, gc_to, code); }
-    else c.codes[gc_to] = (uint8_t)code;
+    atlas_move(c, mr.x, gc_to, code);
     if (sample) {
         atomicAdd(c.st_samp_cnt + e_new, 1u);
         atomicAdd(c.st_samp_code + e_new, (unsigned long long)(code - 1));
@@ -308,23 +309,25 @@ __device__ __forceinline__ void departure_phase2(const Ctx& c, const Slots& S, u
 // ------------------------------------------------------------------ phase drivers
 // `mr_s`: this CTA's move records in shared memory, [mr_j][T]; slots beyond that use c.mr_g.
 
-__device__ __forceinline__ uint32_t phase1(const Ctx& c, const Slots& S, uint32_t k, const Who& me, uint4* mr_s,
-                                           uint32_t mr_j, uint32_t& n_upd) {
-    const uint32_t n_slots = __ldcg(&c.dyn->n_slots);
-    const bool sample = c.p.sample_period && ((k + 1) % c.p.sample_period == 0);
+// `n_slots` must reach the threads without every warp of the grid loading the same word (one
+// L2 slice would serve ~5000 requests in turn): one thread per CTA reads it, see the kernels.
+__device__ __forceinline__ void phase1(const Ctx& c, const Slots& S, uint32_t k, const Who& me, uint4* mr_s,
+                                       uint32_t mr_j, uint32_t n_slots, bool sample, uint32_t& n_upd) {
     for (uint32_t j = 0;; j++) {
         const uint32_t s = me.slot(j);
         if (s >= n_slots) break;
         const uint4 mr = vehicle_phase1(c, S, s, k, sample, n_upd);
         if (j < mr_j) mr_s[j * me.T + me.t] = mr; else stcg4(c.mr_g + s, mr);
     }
-    for (uint32_t q = me.gtid(); q < c.n_queues; q += me.gthreads()) departure_phase1(c, S, q, k);
-    return n_slots;
+    for (uint32_t j = 0;; j++) {
+        const uint32_t q = me.slot(j);
+        if (q - (q & 31u) >= c.n_queues) break;
+        if (q < c.n_queues) departure_phase1(c, S, q, k);
+    }
 }
 
 __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k, const Who& me, const uint4* mr_s,
-                                       uint32_t mr_j, uint32_t n_slots) {
-    const bool sample = c.p.sample_period && ((k + 1) % c.p.sample_period == 0);
+                                       uint32_t mr_j, uint32_t n_slots, bool sample) {
     if (me.gtid() == 0) {
         // every slot handed out in phase 1 takes part from the next step on
         c.dyn->n_slots = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
@@ -337,7 +340,11 @@ __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k,
         const uint4 mr = (j < mr_j) ? mr_s[j * me.T + me.t] : ldcg4(c.mr_g + s);
         vehicle_phase2(c, S, s, k, sample, mr);
     }
-    for (uint32_t q = me.gtid(); q < c.n_queues; q += me.gthreads()) departure_phase2(c, S, q, k, sample);
+    for (uint32_t j = 0;; j++) {
+        const uint32_t q = me.slot(j);
+        if (q - (q & 31u) >= c.n_queues) break;
+        if (q < c.n_queues) departure_phase2(c, S, q, k, sample);
+    }
 }
 
 // order-independent digest of state k+1 (test instrument, not on the timed path).

@@ -45,14 +45,23 @@ __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* red) {
     return red[32];
 }
 
-__device__ __forceinline__ uint32_t sort_rank(const Ctx& c, const Slots& S, const Who& me) {
-    const uint32_t n = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
+// Sort key: the edge, and above it the vehicle's place in the lane-change stagger (readings
+// R10/R14: vehicle id takes its turn when ((k >> 1) + id) % lc_period == 0), so that the warps of
+// one group evaluate lane changes together and the others skip that code.
+__device__ __forceinline__ uint32_t sort_key(const Ctx& c, const uint4& sb) {
+    return (sb.z & (c.sort_groups - 1u)) * c.E + sb.x;
+}
+
+__device__ __forceinline__ uint32_t sort_rank(const Ctx& c, const Slots& S, const Who& me, uint32_t n) {
     for (uint32_t j = 0;; j++) {
         const uint32_t s = me.slot(j);
         if (s >= n) break;
         const uint4 sa = ldcg4(S.A + s);
         uint32_t r = NONE32;
-        if (sa.w & ALIVE) r = atomicAdd(c.hist + __ldcg(&S.B[s].x), 1u);
+        if (sa.w & ALIVE) {
+            const uint4 sb = ldcg4(S.B + s);
+            r = atomicAdd(c.hist + sort_key(c, sb), 1u);
+        }
         c.rank[s] = r;
     }
     // a slot reserved by a waiting departure is not alive and goes away with this compaction
@@ -60,10 +69,11 @@ __device__ __forceinline__ uint32_t sort_rank(const Ctx& c, const Slots& S, cons
     return n;
 }
 
-__device__ __forceinline__ uint32_t edge_share(const Ctx& c, const Who& me) { return (c.E + me.n_cta - 1) / me.n_cta; }
+__device__ __forceinline__ uint32_t n_keys(const Ctx& c) { return c.sort_groups * c.E; }
+__device__ __forceinline__ uint32_t edge_share(const Ctx& c, const Who& me) { return (n_keys(c) + me.n_cta - 1) / me.n_cta; }
 
 __device__ __forceinline__ void sort_partial(const Ctx& c, const Who& me, uint32_t* red) {
-    const uint32_t share = edge_share(c, me), lo = me.cta * share, hi = min(c.E, lo + share);
+    const uint32_t share = edge_share(c, me), lo = me.cta * share, hi = min(n_keys(c), lo + share);
     uint32_t s = 0;
     for (uint32_t e = lo + me.t; e < hi; e += me.T) s += __ldcg(c.hist + e);
     s = block_sum(s, red);
@@ -71,7 +81,7 @@ __device__ __forceinline__ void sort_partial(const Ctx& c, const Who& me, uint32
 }
 
 __device__ __forceinline__ void sort_scan(const Ctx& c, const Who& me, uint32_t* red) {
-    const uint32_t share = edge_share(c, me), lo = me.cta * share, hi = min(c.E, lo + share);
+    const uint32_t share = edge_share(c, me), lo = me.cta * share, hi = min(n_keys(c), lo + share);
     uint32_t mine = 0;
     for (uint32_t b = me.t; b < me.cta; b += me.T) mine += __ldcg(c.partial + b);
     uint32_t run = block_sum(mine, red);                                    // exclusive offset of this CTA
@@ -106,7 +116,7 @@ __device__ __forceinline__ void sort_scatter(const Ctx& c, const Slots& from, co
         const uint32_t r = __ldcg(c.rank + s);
         if (r == NONE32) continue;
         const uint4 sa = ldcg4(from.A + s), sb = ldcg4(from.B + s), sc = ldcg4(from.C + s);
-        const uint32_t d = __ldcg(c.base + sb.x) + r;
+        const uint32_t d = __ldcg(c.base + sort_key(c, sb)) + r;
         stcg4(to.A + d, sa); stcg4(to.B + d, sb); stcg4(to.C + d, sc);
     }
 }
