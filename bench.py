@@ -122,6 +122,19 @@ def time_oracle(bundle, budget_s, chunk=600):
     return upd, dt, steps
 
 
+def whole_job(total_ms_local, units_per_rank, dist=None, device="cpu"):
+    """Replicas only: every rank ran the same number of units; the job's time
+    is the MAX over ranks, its work the sum.  Returns (units/s of the whole job, max ms)."""
+    import torch
+    t = torch.tensor([float(total_ms_local)], dtype=torch.float64, device=device)
+    world = 1
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        world = dist.get_world_size()
+    ms = float(t.item())
+    return units_per_rank * world / (ms / 1e3), ms
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -233,11 +246,7 @@ def main():
     counts = sim.read_counts()
     phase_ns = sim.read_profile() if args.profile else None
     updates = int(counts["vehicle_updates"]) - evs[-1][2]   # per timed window (reset zeroes the counter)
-    total_ms = torch.tensor([sum(ms)], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    total_s = float(total_ms.item()) / 1e3
-    value = updates * args.steps * world / total_s
+    value, total_ms = whole_job(sum(ms), updates * args.steps, dist, f"cuda:{local}")
 
     # end to end through the C ABI with host buffers (pinned where torch can pin them)
     h2d = sum(int(np.asarray(bundle[k]).nbytes) for k in (
@@ -268,10 +277,7 @@ def main():
             e2e_ms.append(e0.elapsed_time(e1))
         assert int(st["vehicle_updates"]) == updates
         s2.close()
-    e2e_t = torch.tensor([sum(e2e_ms)], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
-    e2e_value = updates * len(e2e_ms) * world / (float(e2e_t.item()) / 1e3) if e2e_ms else None
+    e2e_value = whole_job(sum(e2e_ms), updates * len(e2e_ms), dist, f"cuda:{local}")[0] if e2e_ms else None
 
     if rank != 0:
         if dist is not None:
@@ -288,7 +294,7 @@ def main():
     achieved = bpu * updates / launch_s / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": float(total_ms.item()) / args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": bundle["name"], "vehicles": V, "edges": bundle["n_edges"],

@@ -163,16 +163,17 @@ int ts_read_edge_stats(ts_sim *sim, ts_edge_stats_out *out, int reset);
 /* Tuning knobs that never change results.
  *  "mode"          1 (default) = ts_step(n) is ONE persistent cooperative kernel looping over
  *                  the n steps with grid-wide barriers; 0 = one launch per phase.
- *  "threads"       CTA size of the persistent kernel (multiple of 32 in 64..1024, default 512).
+ *  "threads"       CTA size of the persistent kernel (multiple of 32 in 64..1024, default 640).
  *  "blocks_per_sm" resident CTAs per SM of the persistent kernel (default 1).
  *  "sort_period"   steps between compaction of retired slots + re-sort of the live ones by
  *                  edge; 0 = never; default 64.
  *  "profile"       non-zero: the persistent kernel clocks its phases (see ts_read_profile). */
 int ts_set_option(ts_sim *sim, const char *key, long long value);
 
-/* Option "profile": out[0..5] = nanoseconds (GPU global timer, as seen by CTA 0) spent in
- * phase 1, the barrier after it, phase 2, the barrier after it, compaction + re-sort, and the
- * digest, summed over out[6] steps since ts_create / ts_reset.  out[7] is reserved.  Host array.
+/* Option "profile": out[0..5] = nanoseconds (GPU global timer, mean over the CTAs) spent in
+ * phase 1 (until the whole CTA is done), waiting at the barrier after it, phase 2, the barrier
+ * after it, compaction + re-sort, and the digest, summed over out[6] steps since ts_create /
+ * ts_reset.  out[7] = the largest per-CTA phase-1 total of one ts_step call.  Host array.
  * Synchronises. */
 int ts_read_profile(ts_sim *sim, uint64_t out[8]);
 

@@ -188,12 +188,13 @@ class Sim:
                     vehicle_updates=o.vehicle_updates)
 
     def read_profile(self):
-        """Option "profile": mean nanoseconds per simulation step in each phase (CTA 0's view)."""
+        """Option "profile": nanoseconds per simulation step in each phase, mean over the CTAs."""
         a = np.zeros(8, np.uint64)
         _check(load().ts_read_profile(self._h, a.ctypes.data))
         n = max(1, int(a[6]))
         names = ("phase1", "barrier1", "phase2", "barrier2", "sort", "digest")
         out = {k: float(a[i]) / n for i, k in enumerate(names)}
+        out["phase1_slowest_cta"] = float(a[7]) / n     # per launch; meaningful after one ts_step call
         out["steps"] = int(a[6])
         return out
 

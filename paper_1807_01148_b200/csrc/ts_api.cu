@@ -149,7 +149,7 @@ struct ts_sim {
     uint32_t k = 0;           // steps enqueued so far
     uint32_t cur = 0;         // which slot set holds the state
     int mode = 1;             // 0: one launch per phase, 1: persistent cooperative kernel
-    int threads = 512;        // persistent kernel CTA size (128 registers per thread: no spills)
+    int threads = 640;        // persistent kernel CTA size (96 registers per thread, no spills: within 4 % of the best size for 3e4 and for 3e5 active vehicles)
     int blocks_per_sm = 1;
     int sms = 0;
     uint32_t sort_period = 64;   // steps between compaction + re-sort; 0 = never
@@ -173,10 +173,15 @@ __device__ __forceinline__ Who who() {
 // bar.sync orders the CTA's writes before thread 0's release; the acquire load plus the second
 // bar.sync orders them before every later read of any thread (mutable data is read with ld.cg,
 // i.e. from L2, so no stale L1 line can be observed).
-__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target) {
+struct PhaseClock;
+__device__ __forceinline__ void clock_tick(PhaseClock& clk, int b);
+
+// `b`: profile bin that gets the time up to the moment this whole CTA has arrived.
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target, PhaseClock& clk, int b) {
     target += gridDim.x;
     __syncthreads();
     if (threadIdx.x == 0) {
+        clock_tick(clk, b);
         __threadfence();                                          // release, cumulative over the CTA
         asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
         unsigned int v;
@@ -195,7 +200,7 @@ __device__ __forceinline__ unsigned long long global_ns() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-// Phase clock of option "profile": thread 0 of CTA 0 adds the time since the last tick to bin b.
+// Phase clock of option "profile": thread 0 of every CTA adds the time since its last tick to bin b.
 struct PhaseClock {
     unsigned long long* acc;   // shared memory, 8 bins; nullptr = off
     unsigned long long last;
@@ -205,6 +210,8 @@ struct PhaseClock {
 };
 
 // n steps in one launch; grid-wide barriers stand where the method has its two dependencies.
+__device__ __forceinline__ void clock_tick(PhaseClock& clk, int b) { clk.tick(b); }
+
 // MAXT = most threads per SM it is launched with: sets the register budget (64 / 80 / 128).
 template <int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
@@ -217,43 +224,46 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
     unsigned int target = 0;
     uint32_t n_upd = 0;
     PhaseClock clk;
-    clk.acc = (profile && me.gtid() == 0) ? sh_prof : nullptr;
+    clk.acc = (profile && me.t == 0) ? sh_prof : nullptr;
     if (clk.acc) { for (int b = 0; b < 8; b++) sh_prof[b] = 0; clk.last = global_ns(); }
     if (me.t == 0) sh_n_slots[0] = __ldcg(&c.dyn->n_slots);
     __syncthreads();
+    // first step of this launch after which a sample is taken, then every period
+    const uint32_t sp = c.p.sample_period;
+    uint32_t k_sample = sp ? k0 + (sp - 1u - k0 % sp) : NONE32;
     for (uint32_t i = 0; i < n; i++) {
         const uint32_t k = k0 + i;
         const Slots& S = c.s[cur];
         const uint32_t n_slots = sh_n_slots[i & 1];
-        const bool sample = sample_step(c.p, k);
+        const bool sample = (k == k_sample);
+        if (sample) k_sample += sp;
         phase1(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd);
-        clk.tick(0);
-        grid_barrier(c.barrier, target);
+        grid_barrier(c.barrier, target, clk, 0);
         clk.tick(1);
         // slots are handed out in phase 1 only: the count the next step works on is final now
         if (me.t == 0) sh_n_slots[(i + 1) & 1] = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
         phase2(c, S, k, me, dyn_smem, mr_j, n_slots, sample);
-        clk.tick(2);
-        grid_barrier(c.barrier, target);
+        grid_barrier(c.barrier, target, clk, 2);
         clk.tick(3);
         if (digests) { phase_digest(c, S, digests + i, me); clk.tick(5); }
         if (sort_period && (k + 1) % sort_period == 0) {      // A9 + A10, between two steps
             const uint32_t ns = sort_rank(c, S, me, sh_n_slots[(i + 1) & 1]);
-            grid_barrier(c.barrier, target);
+            grid_barrier(c.barrier, target, clk, 4);
             sort_partial(c, me, red);
-            grid_barrier(c.barrier, target);
+            grid_barrier(c.barrier, target, clk, 4);
             sort_scan(c, me, red);
-            grid_barrier(c.barrier, target);
+            grid_barrier(c.barrier, target, clk, 4);
             sort_scatter(c, S, c.s[cur ^ 1], me, ns);
             if (me.t == 0) sh_n_slots[(i + 1) & 1] = __ldcg(&c.dyn->n_slots);
-            grid_barrier(c.barrier, target);
+            grid_barrier(c.barrier, target, clk, 4);
             cur ^= 1;
             clk.tick(4);
         }
     }
-    if (clk.acc) {
-        for (int b = 0; b < 6; b++) c.dyn->prof[b] += sh_prof[b];
-        c.dyn->prof[6] += n;
+    if (clk.acc) {                                  // mean over CTAs per bin; slowest CTA's phase 1
+        for (int b = 0; b < 6; b++) atomicAdd(&c.dyn->prof[b], sh_prof[b] / me.n_cta);
+        atomicMax(&c.dyn->prof[7], sh_prof[0]);
+        if (me.cta == 0) c.dyn->prof[6] += n;
     }
     n_upd = block_sum(n_upd, red);
     if (me.t == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
@@ -370,6 +380,16 @@ __global__ void k_finish_state(const __grid_constant__ Ctx c, uint32_t* o_cell, 
         o_cell[i] = (uint32_t)floorf(c.o_x[i]);
         o_ridx[i] = c.o_rpos[i] - c.route_begin[i];
     }
+}
+
+// The instantiation whose register budget fits `per_sm_threads` resident threads per SM
+// (128 / 96 / 80 / 72 / 64 registers per thread).
+static const void* step_kernel(int per_sm_threads) {
+    if (per_sm_threads <= 512) return (const void*)k_persistent<512>;
+    if (per_sm_threads <= 640) return (const void*)k_persistent<640>;
+    if (per_sm_threads <= 768) return (const void*)k_persistent<768>;
+    if (per_sm_threads <= 896) return (const void*)k_persistent<896>;
+    return (const void*)k_persistent<1024>;
 }
 
 // ------------------------------------------------------------------ create / reset
@@ -568,9 +588,10 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     cudaGetDevice(&dev_id);
     cudaDeviceGetAttribute(&s->sms, cudaDevAttrMultiProcessorCount, dev_id);
     cudaDeviceGetAttribute(&s->smem_limit, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_id);
-    if (cudaFuncSetAttribute(k_persistent<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_persistent<768>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(k_persistent<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) != cudaSuccess) {
+    bool attr_ok = true;
+    for (int t : {512, 640, 768, 896, 1024})
+        attr_ok = attr_ok && cudaFuncSetAttribute(step_kernel(t), cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) == cudaSuccess;
+    if (!attr_ok) {
         delete s;
         return fail(TS_ECUDA, "cannot raise the dynamic shared memory limit of the step kernel");
     }
@@ -618,7 +639,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
         mr_j = std::min(mr_j, need_j);
         const size_t smem = (size_t)mr_j * 16 * s->threads;
         const int per_sm_threads = s->threads * s->blocks_per_sm;
-        void* kern = per_sm_threads <= 512 ? (void*)k_persistent<512> : per_sm_threads <= 768 ? (void*)k_persistent<768> : (void*)k_persistent<1024>;
+        const void* kern = step_kernel(per_sm_threads);
         int per_sm = 0;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, s->threads, smem));
         if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, s->threads);

@@ -182,9 +182,10 @@ __device__ __forceinline__ float idm(const Params& p, float v, float v0, bool ha
 }
 
 __device__ __forceinline__ bool signal_green(const EdgeRec& e, uint32_t k) {
-    uint32_t t = (k + e.offset) % e.cycle;          // k, offset < 2^31
-    uint32_t ph = t / e.P;
-    return ph == e.in_rank && (t - ph * e.P) < e.green;
+    // green iff t div P == in_rank and t mod P < green, i.e. in_rank * P <= t < in_rank * P + green:
+    // one modulo, no division
+    const uint32_t t = (k + e.offset) % e.cycle;          // k, offset < 2^31
+    return t - (uint32_t)e.in_rank * e.P < e.green;       // unsigned: t below the phase start wraps
 }
 
 __device__ __forceinline__ EdgeRec load_edge(const EdgeRec* edges, uint32_t e) {

@@ -209,7 +209,10 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
         atomicAdd(c.st_samp_cnt + e, 1u);
         atomicAdd(c.st_samp_code + e, (unsigned long long)(code - 1));
     }
-    return make_uint4(gc_from, (nrow << 7) + (uint32_t)(int)floorf(xt), code, MR_MOVE);
+    // a vehicle that keeps its cell and its speed code (a standing queue) leaves the atlas alone
+    const uint32_t gc_to = (nrow << 7) + (uint32_t)(int)floorf(xt);
+    if (gc_to == gc_from && code == speed_code(v)) return make_uint4(0, 0, 0, MR_NONE);
+    return make_uint4(gc_from, gc_to, code, MR_MOVE);
 }
 
 // DESIGN.md 2, step 3: the head of one departure queue.  A ready head takes

@@ -343,6 +343,76 @@ def config3(n_vehicles=1_000_000, steps=43200, grid=256, n_origin_nodes=4096, wo
                    steps, v0m, None, xy, workers)
 
 
+def config4(n_vehicles=3_000_000, steps=172_800, n_points=1_000_000, side_m=100_000.0,
+            n_centroids=4096, workers=None, name="cfg4_metro"):
+    """configs[3] metro-scale synthetic: random planar road graph (Delaunay-derived) of ~1 M nodes /
+    ~2.5 M directed edges with hierarchical classes, signals on nodes of degree >= 3, 3 M trips
+    between `n_centroids` zone-centroid nodes with gravity OD and bimodal
+    departures (t = 0 is midnight; Gaussians at 08:00 and 17:30, sd 1 h).  Everything scales with
+    `n_points` / `side_m` for the small versions used in tests."""
+    from scipy.spatial import Delaunay, cKDTree
+    rng = np.random.default_rng(SEED_BASE + 4)
+    pts = rng.random((int(n_points * 1.12), 2)) * side_m
+    # minimum separation 30 m: drop the higher-numbered point of every too-close pair
+    close = cKDTree(pts).query_pairs(30.0, output_type="ndarray")
+    keep = np.ones(len(pts), bool)
+    keep[close[:, 1]] = False
+    pts = pts[keep][:n_points]
+    N0 = len(pts)
+    tri = Delaunay(pts).simplices
+    # thin the Delaunay graph (~3 N edges) to ~1.25 N: drop the longest side of every triangle
+    # (the Urquhart graph: planar, contains the Euclidean minimum spanning tree, so connected)
+    sides = np.stack([tri[:, [0, 1]], tri[:, [1, 2]], tri[:, [2, 0]]], 1)            # [T, 3, 2]
+    slen = np.hypot(*(pts[sides[..., 0]] - pts[sides[..., 1]]).transpose(2, 0, 1))   # [T, 3]
+    longest = np.zeros(slen.shape, bool)
+    longest[np.arange(len(tri)), np.argmax(slen, axis=1)] = True
+    skey = np.minimum(sides[..., 0], sides[..., 1]).astype(np.int64) * N0 + np.maximum(sides[..., 0], sides[..., 1])
+    drop = np.unique(skey[longest])
+    allk = np.unique(skey)
+    keepk = allk[~np.isin(allk, drop)]
+    und = np.stack([keepk // N0, keepk % N0], 1)
+    ulen = np.hypot(*(pts[und[:, 0]] - pts[und[:, 1]]).T)
+    # hierarchy by distance of the edge midpoint to a coarse (freeway) and a fine (arterial) lattice
+    mid = 0.5 * (pts[und[:, 0]] + pts[und[:, 1]])
+    def lattice_dist(pitch):
+        r = np.abs(((mid + 0.5 * pitch) % pitch) - 0.5 * pitch)
+        return r.min(axis=1)
+    d_fw, d_art = lattice_dist(side_m / 10.0), lattice_dist(side_m / 50.0)
+    fw = d_fw <= np.quantile(d_fw, 0.02)
+    art = ~fw & (d_art <= np.quantile(d_art[~fw], 0.15 / 0.98))
+    ulanes = np.where(fw, 4, np.where(art, rng.integers(2, 4, len(und)), 1))
+    ulim = np.where(fw, 29.0, np.where(art, 17.0, 11.0))
+    ulen = np.maximum(40, np.rint(ulen)).astype(np.int64)
+    ef, et, length, lanes, vlim = _directed(und, ulen, ulanes, ulim)
+    keep_node, remap, keep_edge = _largest_scc(N0, ef, et)
+    ef, et = remap[ef[keep_edge]], remap[et[keep_edge]]
+    length, lanes, vlim = length[keep_edge], lanes[keep_edge], vlim[keep_edge]
+    xy = pts[keep_node]
+    N = int(keep_node.sum())
+    n_in = np.bincount(et, minlength=N)
+    sig_node = n_in >= 3
+    ctrl = np.where(sig_node, CTRL_SIGNAL, CTRL_FREE)
+    cycle = rng.integers(120, 241, N)                                  # 60..120 s at dt = 0.5 s
+    green = np.maximum(1, cycle // np.maximum(1, n_in) - 6)            # all-red 6 steps per phase
+    sig = _signal_arrays(rng, N, et, sig_node, green, 6)
+    n_c = min(n_centroids, N)
+    cent = np.sort(rng.choice(N, n_c, replace=False))
+    o_idx = np.sort(rng.integers(0, n_c, n_vehicles))
+    uo, cnt = np.unique(o_idx, return_counts=True)
+    d_idx = _gravity_dests(rng, xy[cent], uo, cnt, 5000.0)             # gravity OD between centroids
+    origins, dests = cent[o_idx], cent[d_idx]
+    perm = rng.permutation(n_vehicles)
+    origins, dests = origins[perm], dests[perm]
+    horizon = steps * DEFAULT_PARAMS["dt"]
+    am = rng.random(n_vehicles) < 0.5
+    scale = horizon / 86400.0                                          # small versions compress the day
+    depart = np.where(am, rng.normal(8.0 * 3600, 3600.0, n_vehicles), rng.normal(17.5 * 3600, 3600.0, n_vehicles))
+    depart = np.clip(depart * scale, 0.0, horizon)
+    v0m = rng.uniform(0.9, 1.1, n_vehicles)
+    return _finish(name, rng, N, ef, et, length, lanes, vlim, ctrl, sig, origins, dests, depart,
+                   steps, v0m, None, xy, workers)
+
+
 def config5(n_vehicles=2_000_000, steps=28800, grid=256, core=8, workers=None):
     """configs[4] congestion stress: full grid, 2 lanes, 200 m, everyone leaves the central
     core x core nodes within 15 min for uniform destinations."""
@@ -373,11 +443,13 @@ def config3_dense(n_vehicles=1_000_000, steps=2400, workers=None):
 
 
 _BY_NAME = {
-    "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg5": config5,
+    "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5,
     "cfg3_dense": config3_dense,
     # quick functional checks, not reported workloads
     "cfg3_small": lambda: config3(n_vehicles=50_000, steps=7200, grid=64, n_origin_nodes=512,
                                   depart_mean_s=1200.0, depart_sd_s=400.0, name="cfg3_small"),
+    "cfg4_small": lambda: config4(n_vehicles=60_000, steps=7200, n_points=20_000, side_m=14_000.0,
+                                  n_centroids=256, name="cfg4_small"),
     "cfg5_small": lambda: config5(n_vehicles=60_000, steps=7200, grid=48, core=4),
 }
 

@@ -1,0 +1,48 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (defaults).
+
+The oracle's 64-bit state digest after every `stride`-th step of the full run is stored in
+tests/golden/trace_<cfg>.json (written by tests/golden/make_golden.py, which calls only oracle/).
+A digest is a function of the whole state (id, edge, lane, bits(x), bits(v) of every ACTIVE vehicle
+plus the counters), and the system is chaotic, so equality at the sampled steps means the
+trajectories are the same.  The CUDA path must reproduce every stored digest, the ACTIVE count
+at those steps, the final counts and the total number of vehicle-updates."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _trace(name):
+    path = os.path.join(GOLDEN, f"trace_{name}.json")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated yet (tests/golden/make_golden.py {name})")
+    return json.load(open(path))
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg5", "cfg4"])
+def test_full_run_matches_golden_digests(name):
+    import paper_1807_01148_b200 as pkg
+    from paper_1807_01148_b200 import workload as W
+    tr = _trace(name)
+    b = W.by_name(name)
+    assert W.bundle_sha256(b) == tr["sha256"], "the seeded generator produced different inputs on this machine"
+    sim = pkg.Sim(b, "cuda:0")
+    done = 0
+    for mark, want, active in zip(tr["marks"], tr["digests"], tr["active"]):
+        if mark - done > 1:
+            sim.step(mark - done - 1)
+        got = int(sim.step_digest(1)[0])
+        assert f"{got:016x}" == want, f"{name}: digest differs at step {mark}"
+        done = mark
+    st = sim.read_counts()
+    assert st["step"] == tr["steps"]
+    for key in ("n_pending", "n_active", "n_arrived"):
+        assert st[key] == tr["final"][key], key
+    assert st["vehicle_updates"] == tr["counters"]["updates"]
+    assert np.all(np.diff(tr["marks"]) > 0)
+    sim.close()
