@@ -47,6 +47,20 @@ def load_workload(name):
         raise SystemExit(str(e))
 
 
+def measured_traffic(name, kernel):
+    """DRAM bytes per launch of `kernel` on workload `name` from the committed ncu --set full
+    capture (profiles/r01_kernel_traffic.csv: workload,kernel,dram_read_bytes,dram_write_bytes)."""
+    path = os.path.join(ROOT, "profiles", "r01_kernel_traffic.csv")
+    try:
+        for line in open(path):
+            f = [t.strip() for t in line.split(",")]
+            if len(f) >= 4 and f[0] == name and f[1] == kernel:
+                return float(f[2]) + float(f[3])
+    except OSError:
+        pass
+    return None
+
+
 def bytes_per_update(name):
     path = os.path.join(ROOT, "tests", "golden", f"trace_{name}.json")
     try:
@@ -175,6 +189,7 @@ def main():
     ap.add_argument("--sort-period", type=int, default=-1, help="steps between compaction + re-sort (tuning)")
     ap.add_argument("--profile", action="store_true", help="clock the phases inside the persistent kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end leg (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -262,7 +277,7 @@ def main():
         pinned[k] = t.numpy().view(bundle[k].dtype)
         pinned["_keep_" + k] = t
     e2e_ms = []
-    for i in range(0 if args.start_step else 1 + max(1, args.steps)):   # diagnostics windows have no e2e leg
+    for i in range(0 if (args.start_step or args.no_e2e) else 1 + max(1, args.steps)):   # diagnostics have no e2e leg
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -308,8 +323,10 @@ def main():
         "gpu_launches": args.steps * (1 if args.mode == 1 else 2 * sim_steps),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                     "kernel": "k_persistent" if args.mode == 1 else "k_intent+k_commit",
+                     "frac": achieved / peak,
+                     "traffic": measured_traffic(args.workload, "k_persistent") if args.mode == 1 and not args.start_step and not args.sim_steps else None,
+                     "peak_source": peak_src,
+                     "kernel": "k_persistent" if args.mode == 1 else "k_phase1+k_phase2",
                      "bytes_per_update": bpu, "scan_cells_per_update": cells, "bytes_source": bsrc,
                      "us_per_sim_step": 1e6 * launch_s / sim_steps},
     }
