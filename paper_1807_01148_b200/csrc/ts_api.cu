@@ -14,7 +14,9 @@
 #include <cstdio>
 #include <cstring>
 #include <numeric>
+#include <atomic>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/trafficsim.h"
@@ -44,6 +46,24 @@ static int fail(int code, const char* fmt, ...) {
 extern "C" const char* ts_last_error(void) { return g_err; }
 extern "C" const char* ts_version(void) {
     return "0.2 (sm_100a, -fmad=false, IEEE div/sqrt, two-plane atlas, persistent step kernel, edge-sorted slots)";
+}
+
+// ------------------------------------------------------------------ host helpers
+
+// fn(begin, end, chunk) over [0, n) on the host cores (ts_create's validation and queue building
+// walk every route entry; on a 1 M-vehicle input that is most of the end-to-end set-up time).
+template <typename F>
+static void parallel_chunks(size_t n, F fn) {
+    unsigned hw = std::thread::hardware_concurrency();
+    const size_t nt = std::max<size_t>(1, std::min<size_t>({(size_t)(hw ? hw : 1), (size_t)16, n / 65536 + 1}));
+    if (nt == 1) { fn((size_t)0, n, (size_t)0); return; }
+    std::vector<std::thread> th;
+    const size_t per = (n + nt - 1) / nt;
+    for (size_t t = 0; t < nt; t++) {
+        const size_t b = std::min(n, t * per), e = std::min(n, b + per);
+        th.emplace_back([=] { fn(b, e, t); });
+    }
+    for (auto& x : th) x.join();
 }
 
 // ------------------------------------------------------------------ layout
@@ -432,13 +452,27 @@ static int validate(const ts_network* net, const ts_routes* rt, const ts_departu
             if (net->sig_offset_steps[h] >= 0x80000000u) return fail(TS_EINVAL, "node %u: offset >= 2^31", h);
         }
     }
-    for (uint32_t i = 0; i < V; i++)
+    // routes: every entry a valid edge, consecutive edges share a node
+    std::atomic<uint32_t> bad_vehicle(0xFFFFFFFFu);
+    parallel_chunks(V, [&](size_t b, size_t e_, size_t) {
+        for (size_t i = b; i < e_; i++)
+            for (uint64_t j = rt->route_off[i]; j < rt->route_off[i + 1]; j++)
+                if (rt->route_edges[j] >= E ||
+                    (j > rt->route_off[i] && net->edge_to[rt->route_edges[j - 1]] != net->edge_from[rt->route_edges[j]])) {
+                    uint32_t cur = bad_vehicle.load();
+                    while ((uint32_t)i < cur && !bad_vehicle.compare_exchange_weak(cur, (uint32_t)i)) {}
+                    return;
+                }
+    });
+    if (bad_vehicle.load() != 0xFFFFFFFFu) {
+        const uint32_t i = bad_vehicle.load();
         for (uint64_t j = rt->route_off[i]; j < rt->route_off[i + 1]; j++) {
             if (rt->route_edges[j] >= E) return fail(TS_EINVAL, "vehicle %u: route edge out of range", i);
             if (j > rt->route_off[i] && net->edge_to[rt->route_edges[j - 1]] != net->edge_from[rt->route_edges[j]])
                 return fail(TS_EINVAL, "vehicle %u: route is not contiguous at position %llu", i,
                             (unsigned long long)(j - rt->route_off[i]));
         }
+    }
     return TS_OK;
 }
 
@@ -540,13 +574,21 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         dep_step[i] = (uint32_t)std::ceil((double)dep->depart_time_s[i] / (double)p->dt);
         route_begin[i] = (uint32_t)rt->route_off[i];
     }
-    std::iota(order.begin(), order.end(), 0u);
+    // counting sort by first edge (ids stay ascending inside an edge), then each queue by
+    // departure step, stable -- i.e. by (edge, departure step, id) -- queues in parallel
     const uint32_t* re = rt->route_edges;
-    std::sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) {
-        const uint32_t ex = re[route_begin[x]], ey = re[route_begin[y]];
-        if (ex != ey) return ex < ey;
-        if (dep_step[x] != dep_step[y]) return dep_step[x] < dep_step[y];
-        return x < y;
+    std::vector<uint32_t> q_begin((size_t)E + 1, 0);
+    for (uint32_t i = 0; i < V; i++) q_begin[re[route_begin[i]] + 1]++;
+    for (uint32_t e = 0; e < E; e++) q_begin[e + 1] += q_begin[e];
+    {
+        std::vector<uint32_t> fill(q_begin.begin(), q_begin.end() - 1);
+        for (uint32_t i = 0; i < V; i++) order[fill[re[route_begin[i]]]++] = i;
+    }
+    parallel_chunks(E, [&](size_t b, size_t e_, size_t) {
+        for (size_t e = b; e < e_; e++)
+            if (q_begin[e + 1] - q_begin[e] > 1)
+                std::stable_sort(order.begin() + q_begin[e], order.begin() + q_begin[e + 1],
+                                 [&](uint32_t x, uint32_t y) { return dep_step[x] < dep_step[y]; });
     });
     // one 32-byte departure record per vehicle in queue order, one 16-byte record per queue
     std::vector<uint4> dep_rec(2 * (size_t)V), queue_rec;
