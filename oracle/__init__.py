@@ -121,6 +121,13 @@ class Oracle:
         out.update(step=step.value, n_pending=npend.value, n_active=nact.value, n_arrived=narr.value)
         return out
 
+    def read_counts(self):
+        """Scalars only."""
+        step = C.c_uint64(); npend = C.c_uint32(); nact = C.c_uint32(); narr = C.c_uint32()
+        lib().orc_read_state(self._h, *([None] * 9), C.addressof(step), C.addressof(npend),
+                             C.addressof(nact), C.addressof(narr))
+        return dict(step=step.value, n_pending=npend.value, n_active=nact.value, n_arrived=narr.value)
+
     def read_edge_stats(self, reset=False):
         E = self.E
         out = dict(entered=np.zeros(E, np.uint32), exited=np.zeros(E, np.uint32),

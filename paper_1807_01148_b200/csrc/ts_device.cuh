@@ -243,22 +243,28 @@ __device__ __forceinline__ Bits160 extract160(const Win& w, int f) {
 // beyond them, none lies within.
 __device__ __forceinline__ int first_occupied(const Win& w, int from, int n) {
     const Bits160 b = extract160(w, from & 127);
-    const unsigned long long lo = ((unsigned long long)b.a1 << 32) | b.a0, hi = ((unsigned long long)b.a3 << 32) | b.a2;
-    int pos = 128 + ((b.a4 & 1u) ? 0 : 64);
-    if (hi) pos = 63 + __ffsll((long long)hi);
-    if (lo) pos = __ffsll((long long)lo) - 1;
+    // branch-free: pick the first non-zero word, then one find-first-set
+    uint32_t word = b.a4 & 1u;
+    int base = 128;
+    if (b.a3) { word = b.a3; base = 96; }
+    if (b.a2) { word = b.a2; base = 64; }
+    if (b.a1) { word = b.a1; base = 32; }
+    if (b.a0) { word = b.a0; base = 0; }
+    const int pos = word ? base + __ffs((int)word) - 1 : 192;
     return pos < n ? from + pos : -1;
 }
 // The last occupied cell among the n cells (n <= 128) that END at cell `last` (the lag vehicle,
 // PAPER.md:400); `w` must hold the chunk before the chunk of `last`, and the chunk of `last`.
 __device__ __forceinline__ int last_occupied(const Win& w, int last, int n) {
     // window bit of `last` is 128 + (last & 127); take the 160 bits that start 128 below it, so
-    // that `last` is bit 128 and the cells below it are bits 127 .. 1
+    // that `last` is bit 128 of them and the cell d behind it is bit 128 - d
     const Bits160 b = extract160(w, last & 127);
-    const unsigned long long lo = (((unsigned long long)b.a1 << 32) | b.a0) & ~1ull, hi = ((unsigned long long)b.a3 << 32) | b.a2;
-    int back = 192;                                   // distance behind `last`
-    if (lo) back = 65 + __clzll((long long)lo);       // bit p of lo is 128 - p cells behind
-    if (hi) back = 1 + __clzll((long long)hi);        // bit p of hi is  64 - p cells behind
+    uint32_t word = b.a0 & ~1u;                        // bit 0 would be 128 cells behind: out of range
+    int top = 31;                                      // bit index (of the 160) of the word's bit 31
+    if (b.a1) { word = b.a1; top = 63; }
+    if (b.a2) { word = b.a2; top = 95; }
+    if (b.a3) { word = b.a3; top = 127; }
+    int back = word ? 128 - (top - __clz((int)word)) : 192;
     if (b.a4 & 1u) back = 0;
     return back < n ? last - back : -1;
 }

@@ -36,8 +36,7 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     // trip 2: edge records and the own-lane window
     const bool last = (e2 == NONE32);
     const EdgeRec E = load_edge(c.edges, e);
-    EdgeRec E2 = E;
-    if (!last) E2 = load_edge(c.edges, e2);
+    const EdgeRec E2 = load_edge(c.edges, last ? e : e2);      // no branch: the last edge stands in for itself
     Win w_own;
     if (fast) w_own = load_win(c.occ, row, (ci + 1) >> 7);
 

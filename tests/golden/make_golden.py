@@ -14,6 +14,9 @@ Stored per config (nothing here ever comes from the CUDA path):
              look at per vehicle-update, used by bench.py for the algorithmic bytes per update
   final      n_pending / n_active / n_arrived after the last step
   seconds    single-thread wall time of the oracle run (context only)
+  complete   false while the run is in progress: the file is rewritten after every stride, so an
+             interrupted run of a very long config (config 4: 5.4e10 vehicle-updates, many hours of
+             the single-threaded oracle) still leaves a usable prefix of digests
 """
 import argparse
 import json
@@ -34,6 +37,8 @@ def run(name, stride):
     orc = Oracle(bundle)
     steps = bundle["steps"]
     marks, digests, active = [], [], []
+    sha = W.bundle_sha256(bundle)
+    path = os.path.join(HERE, f"trace_{name}.json")
     t0 = time.perf_counter()
     done = 0
     while done < steps:
@@ -42,18 +47,17 @@ def run(name, stride):
         done += n
         marks.append(done)
         digests.append(f"{int(d[-1]):016x}")
-        active.append(int(orc.read_state()["n_active"]))
-    secs = time.perf_counter() - t0
-    st = orc.read_state()
-    out = dict(name=bundle["name"], sha256=W.bundle_sha256(bundle), steps=steps, stride=stride,
-               marks=marks, digests=digests, active=active, counters=orc.counters(),
-               final=dict(n_pending=int(st["n_pending"]), n_active=int(st["n_active"]),
-                          n_arrived=int(st["n_arrived"])),
-               seconds=round(secs, 1))
-    path = os.path.join(HERE, f"trace_{name}.json")
-    with open(path, "w") as f:
-        json.dump(out, f, indent=1)
-    print(name, "->", path, f"{secs:.0f} s", out["counters"]["updates"], "updates", flush=True)
+        counts = orc.read_counts()
+        active.append(int(counts["n_active"]))
+        out = dict(name=bundle["name"], sha256=sha, steps=steps, stride=stride, complete=done == steps,
+                   marks=marks, digests=digests, active=active, counters=orc.counters(),
+                   final=dict(n_pending=int(counts["n_pending"]), n_active=int(counts["n_active"]),
+                              n_arrived=int(counts["n_arrived"])),
+                   seconds=round(time.perf_counter() - t0, 1))
+        with open(path + ".tmp", "w") as f:
+            json.dump(out, f, indent=1)
+        os.replace(path + ".tmp", path)
+    print(name, "->", path, f"{out['seconds']:.0f} s", out["counters"]["updates"], "updates", flush=True)
 
 
 if __name__ == "__main__":

@@ -40,7 +40,11 @@ def test_full_run_matches_golden_digests(name):
         assert f"{got:016x}" == want, f"{name}: digest differs at step {mark}"
         done = mark
     st = sim.read_counts()
-    assert st["step"] == tr["steps"]
+    assert st["step"] == tr["marks"][-1]
+    if tr.get("complete", True):
+        assert st["step"] == tr["steps"]
+    # counters of the stored trace are those at its last mark (the whole run, or the prefix of an
+    # oracle run that was still going when the file was committed: see make_golden.py)
     for key in ("n_pending", "n_active", "n_arrived"):
         assert st[key] == tr["final"][key], key
     assert st["vehicle_updates"] == tr["counters"]["updates"]

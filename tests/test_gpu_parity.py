@@ -117,3 +117,39 @@ def test_empty_and_errors(cfg1):
     bad = dict(cfg1); bad["params"] = dict(cfg1["params"], entry_zone_cells=8)
     with pytest.raises(pkg.TsError):
         pkg.Sim(bad, "cuda:0")
+
+
+@pytest.mark.parametrize("params", [
+    dict(lookahead_cells=256, lookback_cells=256),      # scans longer than one 256-cell window
+    dict(lookahead_cells=64, lookback_cells=32),
+    dict(lc_period=3),                                  # stagger is a modulo, not a mask; one sort group
+    dict(lc_period=0),                                  # lane changes off (P5)
+    dict(lc_period=1),                                  # everybody evaluates every step
+    dict(sample_period_steps=1),
+    dict(sample_period_steps=0, insert_clear_cells=16),
+    dict(dt=0.25, a=2.0, b=3.0, T=1.0, s0=1.0, veh_len=4.0, politeness=0.5, lc_threshold=0.2, b_safe=3.0),
+])
+def test_parameter_variants(params):
+    """Every ts_params field away from its default, against the oracle with the same values."""
+    b = small_signal_grid(seed=11, n_vehicles=900, steps=900)
+    b = dict(b, params=dict(b["params"], **params))
+    _compare(b, 900, 1)
+
+
+def test_degenerate_inputs():
+    import paper_1807_01148_b200 as pkg
+    from paper_1807_01148_b200 import workload as W
+    # no vehicles at all: steps run, nothing happens
+    empty = corridor(departs=())
+    sim = pkg.Sim(empty, "cuda:0")
+    sim.step(50)
+    st = sim.read_state()
+    assert st["step"] == 50 and st["n_active"] == 0 and st["vehicle_updates"] == 0 and len(st["x"]) == 0
+    assert sim.read_edge_stats()["n_samples"] == 0
+    sim.close()
+    # one-edge routes (arrive on the edge they start on), 8 lanes, the shortest and a very long edge
+    _compare(corridor(n_edges=3, length=16, lanes=8, vlim=9.0, departs=np.arange(40) * 1.0, route_len=1,
+                      params=dict(entry_zone_cells=12)), 300, 1)
+    _compare(corridor(n_edges=1, length=65535, lanes=3, vlim=29.0, departs=np.arange(200) * 0.5), 1500, 1)
+    # everybody wants the same cell at the same time: 300 vehicles, one origin edge, one departure time
+    _compare(corridor(n_edges=4, length=120, lanes=2, vlim=13.0, departs=np.zeros(300), ctrl=W.CTRL_PRIORITY), 1200, 1)
