@@ -166,7 +166,8 @@ int ts_read_edge_stats(ts_sim *sim, ts_edge_stats_out *out, int reset);
  *  "threads"       CTA size of the persistent kernel (multiple of 32 in 64..1024, default 640).
  *  "blocks_per_sm" resident CTAs per SM of the persistent kernel (default 1).
  *  "sort_period"   steps between compaction of retired slots + re-sort of the live ones by
- *                  edge; 0 = never; default 64.
+ *                  edge; 0 = never; default 128 (256 on networks
+ *                  with more than 4 M sort keys).
  *  "profile"       non-zero: the persistent kernel clocks its phases (see ts_read_profile). */
 int ts_set_option(ts_sim *sim, const char *key, long long value);
 

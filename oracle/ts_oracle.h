@@ -17,10 +17,15 @@
  * every neighbour by an O(V^2) search over raw (edge, lane, x) as a second, independent
  * route to the same answer.
  *
- * Parity pins (tests/test_oracle_pins.py): P1 lone-vehicle closed form, P2 platoon
- * equilibrium gap, P3 standing queue, I1-I8 invariants, P4 brute force, P5 degenerate cases.
- * PARITY UNPINNED against the outside world (pinned oracle<->GPU only): the MOBIL
- * incentive values, hold-at-line behaviour and departure ordering (SURVEY.md:425-426).
+ * Parity pins (tests/test_oracle_pins.py, test_oracle_invariants.py, test_oracle_scenarios.py):
+ * P1 lone-vehicle closed form, P2 platoon equilibrium gap, P3 standing queue, I1-I8 invariants,
+ * P4 brute force, P5 degenerate cases; scenario pins re-derived in fp64 from the rule text: the
+ * discretionary lane-change decision with an empty target lane (incentive vs threshold on every
+ * turn), gap acceptance at the moment of every change, hold-at-line after a lost claim with the
+ * lowest id first, departure order and entry clearance.
+ * PARITY UNPINNED against the outside world (pinned oracle<->GPU only): the VALUE of the MOBIL
+ * politeness term (new follower's loss) and of the mandatory-change threshold; these have no
+ * statement in the paper beyond PAPER.md:399-400 to pin them to.
  */
 #ifndef TS_ORACLE_H
 #define TS_ORACLE_H
