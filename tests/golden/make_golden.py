@@ -32,13 +32,13 @@ from oracle import Oracle                                    # noqa: E402
 from paper_1807_01148_b200 import workload as W              # noqa: E402
 
 
-def run(name, stride):
+def run(name, stride, suffix=""):
     bundle = W.by_name(name)
     orc = Oracle(bundle)
     steps = bundle["steps"]
     marks, digests, active = [], [], []
     sha = W.bundle_sha256(bundle)
-    path = os.path.join(HERE, f"trace_{name}.json")
+    path = os.path.join(HERE, f"trace_{name}{suffix}.json")
     t0 = time.perf_counter()
     done = 0
     while done < steps:
@@ -64,6 +64,7 @@ if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("configs", nargs="+")
     ap.add_argument("--stride", type=int, default=600)
+    ap.add_argument("--suffix", default="", help="write trace_<cfg><suffix>.json (a second, incremental run beside a long one)")
     a = ap.parse_args()
     for c in a.configs:
-        run(c, a.stride)
+        run(c, a.stride, a.suffix)

@@ -20,6 +20,8 @@ GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 def _trace(name):
     path = os.path.join(GOLDEN, f"trace_{name}.json")
     if not os.path.exists(path):
+        path = os.path.join(GOLDEN, f"trace_{name}_partial.json")      # prefix of a run still going
+    if not os.path.exists(path):
         pytest.skip(f"{path} not generated yet (tests/golden/make_golden.py {name})")
     return json.load(open(path))
 
