@@ -215,6 +215,12 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
 
 extern __shared__ uint4 dyn_smem[];
 
+// The static record of the first (normally the only) departure queue this thread looks after.
+__device__ __forceinline__ uint4 first_queue_rec(const Ctx& c, const Who& me) {
+    const uint32_t q = me.slot(0);
+    return q < c.n_queues ? __ldg(c.queue_rec + q) : make_uint4(0, 0, 0, 0);
+}
+
 __device__ __forceinline__ unsigned long long global_ns() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -248,6 +254,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
     if (clk.acc) { for (int b = 0; b < 8; b++) sh_prof[b] = 0; clk.last = global_ns(); }
     if (me.t == 0) sh_n_slots[0] = __ldcg(&c.dyn->n_slots);
     __syncthreads();
+    const uint4 qr0 = first_queue_rec(c, me);      // held in registers for the whole launch
     // first step of this launch after which a sample is taken, then every period
     const uint32_t sp = c.p.sample_period;
     uint32_t k_sample = sp ? k0 + (sp - 1u - k0 % sp) : NONE32;
@@ -257,12 +264,12 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
         const uint32_t n_slots = sh_n_slots[i & 1];
         const bool sample = (k == k_sample);
         if (sample) k_sample += sp;
-        phase1(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd);
+        phase1(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd, qr0);
         grid_barrier(c.barrier, target, clk, 0);
         clk.tick(1);
         // slots are handed out in phase 1 only: the count the next step works on is final now
         if (me.t == 0) sh_n_slots[(i + 1) & 1] = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
-        phase2(c, S, k, me, dyn_smem, mr_j, n_slots, sample);
+        phase2(c, S, k, me, dyn_smem, mr_j, n_slots, sample, qr0);
         grid_barrier(c.barrier, target, clk, 2);
         clk.tick(3);
         if (digests) { phase_digest(c, S, digests + i, me); clk.tick(5); }
@@ -298,7 +305,8 @@ __global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, u
     if (threadIdx.x == 0) sh_n = __ldcg(&c.dyn->n_slots);
     __syncthreads();
     const uint32_t n_slots = sh_n;
-    phase1(c, c.s[cur], k, who(), nullptr, 0, n_slots, sample_step(c.p, k), n_upd);
+    const Who me = who();
+    phase1(c, c.s[cur], k, me, nullptr, 0, n_slots, sample_step(c.p, k), n_upd, first_queue_rec(c, me));
     if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n_slots;   // phase 2 overwrites dyn->n_slots
     n_upd = block_sum(n_upd, red);
     if (threadIdx.x == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
@@ -307,7 +315,8 @@ __global__ void __launch_bounds__(256) k_phase2(const __grid_constant__ Ctx c, u
     __shared__ uint32_t sh_n;
     if (threadIdx.x == 0) sh_n = __ldcg(&c.dyn->pad);
     __syncthreads();
-    phase2(c, c.s[cur], k, who(), nullptr, 0, sh_n, sample_step(c.p, k));
+    const Who me = who();
+    phase2(c, c.s[cur], k, me, nullptr, 0, sh_n, sample_step(c.p, k), first_queue_rec(c, me));
 }
 __global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, uint32_t cur, unsigned long long* out) {
     phase_digest(c, c.s[cur], out, who());   // test instrument: may read the slot count per thread

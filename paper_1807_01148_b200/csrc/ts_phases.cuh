@@ -217,8 +217,8 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
 // DESIGN.md 2, step 3: the head of one departure queue.  A ready head takes
 // a slot (kept as the queue's reservation until it wins) and writes its not-yet-alive state right
 // away; phase 2 only flips it alive if it holds the lane claim.
-__device__ __forceinline__ void departure_phase1(const Ctx& c, const Slots& S, uint32_t q, uint32_t k) {
-    const uint4 qr = __ldg(c.queue_rec + q);           // { row, lane_base, end, edge }
+__device__ __forceinline__ void departure_phase1(const Ctx& c, const Slots& S, uint32_t q, uint32_t k, const uint4 qr) {
+    // qr = queue_rec[q] = { row, lane_base, end, edge }
     const uint4 qs = ldcg4(c.queue_state + q);         // { head, dep step of the head, reserved slot, - }
     uint4 cand = make_uint4(NONE32, 0, 0, 0);
     if (qs.x < qr.z && qs.y <= k) {
@@ -259,9 +259,12 @@ __device__ __forceinline__ void vehicle_phase2(const Ctx& c, const Slots& S, uin
     // MR_CROSS: one trip for everything
     const uint4 sa = ldcg4(S.A + slot), sb = ldcg4(S.B + slot), sc = ldcg4(S.C + slot);
     const uint4 c0 = ldcg4(c.cr + 2 * (size_t)slot), c1 = ldcg4(c.cr + 2 * (size_t)slot + 1);
-    const unsigned long long w = claim_word(k, sb.z);
+    // both claim words are fetched with the slot state, whether the node claim is needed or not:
+    // a load issued only once `w` is known would be a second trip
     const unsigned long long wl = __ldcg(c.lane_claim + mr.y);
-    const unsigned long long wn = (mr.z != NONE32) ? __ldcg(c.node_claim + mr.z) : w;
+    const unsigned long long wn_raw = __ldcg(c.node_claim + (mr.z != NONE32 ? mr.z : 0u));
+    const unsigned long long w = claim_word(k, sb.z);
+    const unsigned long long wn = (mr.z != NONE32) ? wn_raw : w;
     const uint32_t e = sb.x, e2 = sb.y, l = sa.w & 0xFu, k1 = k + 1;
     float xn, vn;
     uint32_t gc_to, e_new;
@@ -293,11 +296,14 @@ __device__ __forceinline__ void vehicle_phase2(const Ctx& c, const Slots& S, uin
 }
 
 // DESIGN.md 2, step 4 (departures): the winning queue head becomes ACTIVE at x = 0, v = 0, lane 0.
-__device__ __forceinline__ void departure_phase2(const Ctx& c, const Slots& S, uint32_t q, uint32_t k, bool sample) {
+// `qr` = queue_rec[q]: static, kept in a register by the persistent kernel, so that the candidate
+// and the claim word are ONE trip.
+__device__ __forceinline__ void departure_phase2(const Ctx& c, const Slots& S, uint32_t q, uint32_t k, bool sample,
+                                                 const uint4 qr) {
     const uint4 cand = __ldcg(c.queue_cand + q);       // { id, slot, head, dep step of the next }
+    const unsigned long long claim = __ldcg(c.lane_claim + qr.y);
     if (cand.x == NONE32) return;
-    const uint4 qr = __ldg(c.queue_rec + q);
-    if (__ldcg(c.lane_claim + qr.y) != claim_word(k, cand.x)) return;   // the slot stays dead
+    if (claim != claim_word(k, cand.x)) return;        // the slot stays reserved
     const uint32_t k1 = k + 1;
     stcg4(S.A + cand.y, make_uint4(0u, 0u, qr.x, ALIVE));
     c.o_status[cand.x] = 1; c.o_insert[cand.x] = k1;
@@ -314,7 +320,7 @@ __device__ __forceinline__ void departure_phase2(const Ctx& c, const Slots& S, u
 // `n_slots` must reach the threads without every warp of the grid loading the same word (one
 // L2 slice would serve ~5000 requests in turn): one thread per CTA reads it, see the kernels.
 __device__ __forceinline__ void phase1(const Ctx& c, const Slots& S, uint32_t k, const Who& me, uint4* mr_s,
-                                       uint32_t mr_j, uint32_t n_slots, bool sample, uint32_t& n_upd) {
+                                       uint32_t mr_j, uint32_t n_slots, bool sample, uint32_t& n_upd, const uint4 qr0) {
     for (uint32_t j = 0;; j++) {
         const uint32_t s = me.slot(j);
         if (s >= n_slots) break;
@@ -324,12 +330,12 @@ __device__ __forceinline__ void phase1(const Ctx& c, const Slots& S, uint32_t k,
     for (uint32_t j = 0;; j++) {
         const uint32_t q = me.slot(j);
         if (q - (q & 31u) >= c.n_queues) break;
-        if (q < c.n_queues) departure_phase1(c, S, q, k);
+        if (q < c.n_queues) departure_phase1(c, S, q, k, j == 0 ? qr0 : __ldg(c.queue_rec + q));
     }
 }
 
 __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k, const Who& me, const uint4* mr_s,
-                                       uint32_t mr_j, uint32_t n_slots, bool sample) {
+                                       uint32_t mr_j, uint32_t n_slots, bool sample, const uint4 qr0) {
     if (me.gtid() == 0) {
         // every slot handed out in phase 1 takes part from the next step on
         c.dyn->n_slots = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
@@ -345,7 +351,7 @@ __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k,
     for (uint32_t j = 0;; j++) {
         const uint32_t q = me.slot(j);
         if (q - (q & 31u) >= c.n_queues) break;
-        if (q < c.n_queues) departure_phase2(c, S, q, k, sample);
+        if (q < c.n_queues) departure_phase2(c, S, q, k, sample, j == 0 ? qr0 : __ldg(c.queue_rec + q));
     }
 }
 
