@@ -28,7 +28,7 @@ const char *orc_last_error(void) { return g_err; }
 
 struct orc_sim {
     orc_params p;
-    float K;                       /* 2*sqrtf(a*b), fp32, computed once */
+    float Kinv;                    /* 1 / (2*sqrtf(a*b)), fp32, computed once (reading R27) */
     uint32_t N, E, V;
     /* network */
     uint32_t *edge_from, *edge_to, *edge_len;
@@ -94,17 +94,21 @@ float orc_speed_decode(uint8_t code) { return (float)((int)code - 1) * 0.25f; }
 
 /* Intelligent Driver Model, Eq. 7 (readings R1, R2, R8):
  *   dv/dt = a * ( 1 - (v/v0)^4 - ((s0 + max(0, T v + v dv / (2 sqrt(a b)))) / max(s, 0.5))^2 )
- * with s the net gap to the car ahead and dv = v - v_leader. */
+ * with s the net gap to the car ahead and dv = v - v_leader.
+ * Reading R27: the two quotients whose divisor does not depend on the traffic are
+ * formed with a reciprocal rounded once -- v/v0 as v * (1/v0), v dv/(2 sqrt(ab)) as (v dv) * (1/K)
+ * -- each still one rounding per written operation; s* / s stays a division. */
 static float idm(const orc_sim *S, float v, float v0, int has, float s, float dv) {
     const orc_params *p = &S->p;
-    float r = v / v0;
+    float rinv = 1.0f / v0;
+    float r = v * rinv;
     float r2 = r * r;
     float r4 = r2 * r2;
     float fr = 1.0f - r4;
     if (!has) return p->a * fr;
     float t = v * p->T;
     float u = v * dv;
-    float w = u / S->K;
+    float w = u * S->Kinv;
     t = t + w;
     t = fmaxf(t, 0.0f);
     float ss = p->s0 + t;
@@ -119,7 +123,7 @@ float orc_idm(const orc_params *p, float v, float v0, int has_leader, float s, f
     orc_sim tmp;
     tmp.p = *p;
     float ab = p->a * p->b;
-    tmp.K = 2.0f * sqrtf(ab);
+    { float K = 2.0f * sqrtf(ab); tmp.Kinv = 1.0f / K; }
     return idm(&tmp, v, v0, has_leader, s, dv);
 }
 
@@ -214,7 +218,7 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
 
     orc_sim *S = (orc_sim *)xcalloc(1, sizeof *S);
     S->p = *p;
-    { float ab = p->a * p->b; S->K = 2.0f * sqrtf(ab); }
+    { float ab = p->a * p->b; float K = 2.0f * sqrtf(ab); S->Kinv = 1.0f / K; }
     S->N = n_nodes; S->E = n_edges; S->V = n_vehicles;
     uint32_t N = n_nodes, E = n_edges, V = n_vehicles;
     S->edge_from = xdup(edge_from, E, 4); S->edge_to = xdup(edge_to, E, 4);

@@ -3,7 +3,8 @@
  *
  * A plain, slow, single-threaded CPU restatement of the per-vehicle traffic
  * microsimulation of arxiv 1807.01148 (sections 6.3.2-6.3.3), following
- * SURVEY.md section 8(c) step by step (readings R1-R22 are listed in DESIGN.md).
+ * SURVEY.md section 8(c) step by step (readings R1-R27 are listed in DESIGN.md; R27 fixes the
+ * rounding order of two quotients inside Eq. 7).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
  * may load this library.  It shares no code, header, table or helper with the CUDA path

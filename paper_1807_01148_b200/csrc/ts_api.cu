@@ -491,7 +491,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     Params& q = c.p;
     q.dt = p->dt; q.a = p->a; q.b = p->b; q.T = p->T; q.s0 = p->s0; q.len = p->veh_len;
     q.b_safe = p->b_safe; q.politeness = p->politeness; q.lc_threshold = p->lc_threshold;
-    { volatile float ab = p->a * p->b; volatile float r = sqrtf(ab); q.K = 2.0f * r; }
+    { volatile float ab = p->a * p->b; volatile float r = sqrtf(ab); volatile float K = 2.0f * r; q.Kinv = 1.0f / K; }
     { volatile float h = 0.5f * p->a; q.half_a_dt = h * p->dt; }
     q.a_dt = p->a * p->dt;
     q.entry_zone_f = (float)p->entry_zone_cells;

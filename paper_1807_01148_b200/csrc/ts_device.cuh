@@ -70,7 +70,7 @@ struct Dyn {
 
 struct Params {
     float dt, a, b, T, s0, len, b_safe, politeness, lc_threshold;
-    float K;               // 2*sqrtf(a*b), computed once on the host in fp32
+    float Kinv;            // 1 / (2*sqrtf(a*b)), computed once on the host in fp32 (reading R27)
     float half_a_dt;       // (0.5f*a)*dt   (E4)
     float a_dt;            // a*dt          (E5)
     float entry_zone_f;
@@ -160,7 +160,8 @@ __device__ __forceinline__ float speed_decode(uint32_t code) { return (float)((i
 
 // Eq. 7: a*(1 - (v/v0)^4 - (s*/s)^2), s* = s0 + max(0, vT + v dv / (2 sqrt(ab))).
 __device__ __forceinline__ float idm_free(float v, float v0) {
-    float r = v / v0;
+    float rinv = __frcp_rn(v0);                     // the correctly rounded 1.0f / v0 (reading R27)
+    float r = v * rinv;
     float r2 = r * r;
     float r4 = r2 * r2;
     return 1.0f - r4;
@@ -170,7 +171,7 @@ __device__ __forceinline__ float idm(const Params& p, float v, float v0, bool ha
     if (!has) return p.a * fr;
     float t = v * p.T;
     float u = v * dv;
-    float w = u / p.K;
+    float w = u * p.Kinv;
     t = t + w;
     t = fmaxf(t, 0.0f);
     float ss = p.s0 + t;
