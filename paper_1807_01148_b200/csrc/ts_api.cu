@@ -110,7 +110,10 @@ struct Layout {
 };
 
 // Sizes only (what ts_query_workspace may look at).
-static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_params* prm, Layout& L) {
+// `first_edge` (optional): receives each vehicle's first route edge, so that ts_create gathers
+// them from the route table (one random read per vehicle into hundreds of MB) only once.
+static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_params* prm, Layout& L,
+                      std::vector<uint32_t>* first_edge = nullptr) {
     if (!net || !rt || !prm) return fail(TS_EINVAL, "null argument");
     // the re-sort groups vehicles by their place in the lane-change stagger when that is a mask
     const uint32_t lcp = prm->lc_period;
@@ -131,14 +134,29 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_param
     // a cell is addressed by one 32-bit index (row * 128 + cell)
     if (chunks + 2 >= (1ull << 25)) return fail(TS_EINVAL, "atlas larger than 2^32 cells");
     L.atlas_chunks = chunks; L.n_lanes = lanes;
+    std::vector<uint32_t> fe_local;
+    std::vector<uint32_t>& fe = first_edge ? *first_edge : fe_local;
+    fe.assign(L.V, 0);
+    std::atomic<uint32_t> bad(0xFFFFFFFFu);
+    parallel_chunks(L.V, [&](size_t b, size_t e_, size_t) {
+        for (size_t i = b; i < e_; i++) {
+            if (rt->route_off[i + 1] <= rt->route_off[i] || rt->route_edges[rt->route_off[i]] >= L.E) {
+                uint32_t cur = bad.load();
+                while ((uint32_t)i < cur && !bad.compare_exchange_weak(cur, (uint32_t)i)) {}
+                return;
+            }
+            fe[i] = rt->route_edges[rt->route_off[i]];
+        }
+    });
+    if (bad.load() != 0xFFFFFFFFu) {
+        const uint32_t i = bad.load();
+        if (rt->route_off[i + 1] <= rt->route_off[i]) return fail(TS_EINVAL, "vehicle %u: empty route", i);
+        return fail(TS_EINVAL, "vehicle %u: route edge %u out of range", i, rt->route_edges[rt->route_off[i]]);
+    }
     std::vector<uint8_t> is_origin(L.E, 0);
     uint32_t q = 0;
-    for (uint32_t i = 0; i < L.V; i++) {
-        if (rt->route_off[i + 1] <= rt->route_off[i]) return fail(TS_EINVAL, "vehicle %u: empty route", i);
-        uint32_t e = rt->route_edges[rt->route_off[i]];
-        if (e >= L.E) return fail(TS_EINVAL, "vehicle %u: route edge %u out of range", i, e);
-        if (!is_origin[e]) { is_origin[e] = 1; q++; }
-    }
+    for (uint32_t i = 0; i < L.V; i++)
+        if (!is_origin[fe[i]]) { is_origin[fe[i]] = 1; q++; }
     L.Q = q;
     // a vehicle takes one slot when it departs; a queue head that is ready but has not won its
     // lane yet holds one reserved slot, which a compaction may drop (then it takes a new one)
@@ -543,7 +561,8 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(TS_ECUDA, "no CUDA device: this library has no CPU fallback");
     Layout L;
-    int rc = plan_sizes(net, rt, p, L);
+    std::vector<uint32_t> first_edge;
+    int rc = plan_sizes(net, rt, p, L, &first_edge);
     if (rc) return rc;
     if ((uint64_t)L.groups * L.E >= 0xFFFFFFF0ull) L.groups = 1;
     if ((rc = validate(net, rt, dep, p))) return rc;
@@ -587,11 +606,11 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     // departure step, stable -- i.e. by (edge, departure step, id) -- queues in parallel
     const uint32_t* re = rt->route_edges;
     std::vector<uint32_t> q_begin((size_t)E + 1, 0);
-    for (uint32_t i = 0; i < V; i++) q_begin[re[route_begin[i]] + 1]++;
+    for (uint32_t i = 0; i < V; i++) q_begin[first_edge[i] + 1]++;
     for (uint32_t e = 0; e < E; e++) q_begin[e + 1] += q_begin[e];
     {
         std::vector<uint32_t> fill(q_begin.begin(), q_begin.end() - 1);
-        for (uint32_t i = 0; i < V; i++) order[fill[re[route_begin[i]]]++] = i;
+        for (uint32_t i = 0; i < V; i++) order[fill[first_edge[i]]++] = i;
     }
     parallel_chunks(E, [&](size_t b, size_t e_, size_t) {
         for (size_t e = b; e < e_; e++)
