@@ -153,3 +153,31 @@ def test_degenerate_inputs():
     _compare(corridor(n_edges=1, length=65535, lanes=3, vlim=29.0, departs=np.arange(200) * 0.5), 1500, 1)
     # everybody wants the same cell at the same time: 300 vehicles, one origin edge, one departure time
     _compare(corridor(n_edges=4, length=120, lanes=2, vlim=13.0, departs=np.zeros(300), ctrl=W.CTRL_PRIORITY), 1200, 1)
+
+
+def test_chunking_across_sort_boundaries():
+    """ts_step(n) in uneven pieces: the host must know which slot set is current after every
+    launch, whatever number of re-sorts fell inside it (sort period 7: launches of 1, 6, 7, 8, 13
+    and 20 steps end just before, on and just after a boundary)."""
+    import paper_1807_01148_b200 as pkg
+    from oracle import Oracle
+    b = small_signal_grid(seed=5, n_vehicles=700, steps=600)
+    want = Oracle(b).step(600, digests=True)
+    for mode in (1, 0):
+        sim = pkg.Sim(b, "cuda:0", mode=mode)
+        sim.set_option("sort_period", 7)
+        got, pieces, i = [], (1, 6, 7, 8, 13, 20, 1, 1, 5), 0
+        while len(got) < 600:
+            n = min(pieces[i % len(pieces)], 600 - len(got))
+            if i % 3 == 2:
+                sim.step(n - 1) if n > 1 else None          # plain steps, then a digest for the last
+                got.extend([None] * (n - 1))
+                got.append(int(sim.step_digest(1)[0]))
+            else:
+                got.extend(int(d) for d in sim.step_digest(n))
+            i += 1
+        bad = [k for k, d in enumerate(got) if d is not None and d != int(want[k])]
+        assert not bad, f"mode {mode}: first mismatch at step {bad[0] + 1}"
+        st = sim.read_state()
+        assert st["step"] == 600
+        sim.close()
