@@ -14,6 +14,9 @@ Stored per config (nothing here ever comes from the CUDA path):
              look at per vehicle-update, used by bench.py for the algorithmic bytes per update
   final      n_pending / n_active / n_arrived after the last step
   seconds    single-thread wall time of the oracle run (context only)
+  edge_stats sums of the oracle's per-edge accumulators at the last mark (entered, exited,
+             exit_steps_sum, sample_count_sum, sample_speedcode_sum, n_samples) and a position-weighted
+             checksum of each: the digests do not cover these
   complete   false while the run is in progress: the file is rewritten after every stride, so an
              interrupted run of a very long config (config 4: 5.4e10 vehicle-updates, many hours of
              the single-threaded oracle) still leaves a usable prefix of digests
@@ -23,6 +26,8 @@ import json
 import os
 import sys
 import time
+
+import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
@@ -49,7 +54,13 @@ def run(name, stride, suffix=""):
         digests.append(f"{int(d[-1]):016x}")
         counts = orc.read_counts()
         active.append(int(counts["n_active"]))
+        es = orc.read_edge_stats()
+        w = np.arange(1, orc.E + 1, dtype=np.uint64)
+        edge_stats = {k: [int(np.asarray(v, np.uint64).sum()), int((np.asarray(v, np.uint64) * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF))]
+                      for k, v in es.items() if k != "n_samples"}
+        edge_stats["n_samples"] = int(es["n_samples"])
         out = dict(name=bundle["name"], sha256=sha, steps=steps, stride=stride, complete=done == steps,
+                   edge_stats=edge_stats,
                    marks=marks, digests=digests, active=active, counters=orc.counters(),
                    final=dict(n_pending=int(counts["n_pending"]), n_active=int(counts["n_active"]),
                               n_arrived=int(counts["n_arrived"])),

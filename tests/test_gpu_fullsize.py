@@ -50,5 +50,16 @@ def test_full_run_matches_golden_digests(name):
     for key in ("n_pending", "n_active", "n_arrived"):
         assert st[key] == tr["final"][key], key
     assert st["vehicle_updates"] == tr["counters"]["updates"]
+    if "edge_stats" in tr:                  # A11 and the edge counters: not covered by the digests
+        es = sim.read_edge_stats()
+        w = np.arange(1, len(es["entered"]) + 1, dtype=np.uint64)
+        assert int(es["n_samples"]) == tr["edge_stats"]["n_samples"]
+        for key, pair in tr["edge_stats"].items():
+            if key == "n_samples":
+                continue
+            total, weighted = pair
+            v = np.asarray(es[key], np.uint64)
+            assert int(v.sum()) == total, key
+            assert int((v * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF)) == weighted, key
     assert np.all(np.diff(tr["marks"]) > 0)
     sim.close()
