@@ -34,8 +34,11 @@ UNIT = "vehicle-updates/s"
 # Algorithmic bytes per vehicle-update:
 #   32 (state read) + 8 (x, v written) + S_own + S_lc + 2 (atlas erase + store)
 # with S_own / S_lc = mean atlas cells scanned per update in the own lane (+ next edge) and in
-# the lane-change target lane, taken from the oracle's work counters for the full run of the
-# config (tests/golden/trace_<cfg>.json, written by tests/golden/make_golden.py).
+# the lane-change target lane, taken from the oracle's work counters in the stored trace of the
+# config (tests/golden/trace_<cfg>[_partial].json, written by tests/golden/make_golden.py): the
+# whole run where the oracle has finished it, else the prefix it has reached -- the JSON line says
+# which in roofline.bytes_source, and the figure moves with the prefix (cells scanned per update
+# fall as traffic builds up).
 SCAN_CELLS_FALLBACK = {"cfg1": 87.3 + 12.9, "cfg2": 11.4 + 2.7, "cfg3": 60.0, "cfg5": 30.0}
 
 
