@@ -19,7 +19,7 @@ _PARAM_FIELDS = [
     ("lc_threshold", C.c_float), ("mand_dist_default", C.c_float),
     ("lookahead_cells", C.c_uint32), ("lookback_cells", C.c_uint32), ("lc_period", C.c_uint32),
     ("entry_zone_cells", C.c_uint32), ("insert_clear_cells", C.c_uint32),
-    ("sample_period_steps", C.c_uint32),
+    ("sample_period_steps", C.c_uint32), ("emissions", C.c_uint32),
 ]
 
 
@@ -51,6 +51,12 @@ def lib():
         L.orc_read_state.argtypes = [C.c_void_p] * 14
         L.orc_read_edge_stats.restype = None
         L.orc_read_edge_stats.argtypes = [C.c_void_p] * 7 + [C.c_int]
+        L.orc_read_emissions.restype = None
+        L.orc_read_emissions.argtypes = [C.c_void_p] * 3
+        L.orc_co_rate.restype = C.c_float
+        L.orc_co_rate.argtypes = [C.c_float]
+        L.orc_fuel_rate.restype = C.c_float
+        L.orc_fuel_rate.argtypes = [C.c_float, C.c_float]
         L.orc_get_counters.restype = None
         L.orc_get_counters.argtypes = [C.c_void_p, C.POINTER(OrcCounters)]
         L.orc_destroy.restype = None
@@ -73,7 +79,7 @@ def lib():
 def make_params(d) -> OrcParams:
     p = OrcParams()
     for name, _ in _PARAM_FIELDS:
-        setattr(p, name, d[name])
+        setattr(p, name, d.get(name, 0) if name == "emissions" else d[name])
     return p
 
 
@@ -139,6 +145,12 @@ class Oracle:
         out["n_samples"] = ns.value
         return out
 
+    def read_emissions(self):
+        """Per-vehicle grams of CO (Eq. 8) and millilitres of fuel (Eq. 9) since step 0."""
+        out = dict(co_g=np.zeros(self.V, np.float32), fuel_ml=np.zeros(self.V, np.float32))
+        lib().orc_read_emissions(self._h, _ptr(out["co_g"]), _ptr(out["fuel_ml"]))
+        return out
+
     def counters(self):
         c = OrcCounters()
         lib().orc_get_counters(self._h, C.byref(c))
@@ -154,6 +166,14 @@ class Oracle:
             self.close()
         except Exception:
             pass
+
+
+def co_rate(v):
+    return float(lib().orc_co_rate(v))
+
+
+def fuel_rate(v, acc):
+    return float(lib().orc_fuel_rate(v, acc))
 
 
 def idm(params, v, v0, has_leader, s, dv):

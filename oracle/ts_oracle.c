@@ -72,6 +72,7 @@ struct orc_sim {
     /* outputs */
     uint32_t *entered, *exited, *sample_count_sum;
     uint64_t *exit_steps_sum, *sample_speedcode_sum;
+    float *co_g, *fuel_ml;         /* [V] section 6.3.4 accumulators */
     uint32_t n_samples;
     uint64_t k;                    /* current step */
     uint32_t n_pending, n_active, n_arrived;
@@ -125,6 +126,50 @@ float orc_idm(const orc_params *p, float v, float v0, int has_leader, float s, f
     float ab = p->a * p->b;
     { float K = 2.0f * sqrtf(ab); tmp.Kinv = 1.0f / K; }
     return idm(&tmp, v, v0, has_leader, s, dv);
+}
+
+/* CO emission rate, Eq. 8 (Stein and Walker 2003):
+ *   P = -0.064 + 0.0056 v_m + 0.00026 (v_m - 50)^2      [g/s], v_m = speed in miles per hour.
+ * v is in m/s; 1 m/s = 3600/1609.344 mph = 2.2369363 mph (reading R28: the fp32 nearest to that
+ * ratio).  Evaluated left to right, one rounding per written operation. */
+float orc_co_rate(float v) {
+    float vm = v * 2.2369363f;
+    float P = 0.0056f * vm;
+    P = -0.064f + P;
+    float d = vm - 50.0f;
+    float d2 = d * d;
+    float q = 0.00026f * d2;
+    P = P + q;
+    return P;
+}
+
+/* Fuel consumption rate, Eq. 9 (Akcelik 1989):
+ *   f = 0.666 + 0.072 (0.269 v + 0.0171 v^2 + 0.000672 v^3 + 1.680 a v + P_ea)   [mL/s],
+ *   P_ea = 0.79296 a^2 v for a > 0 (else 0), v in m/s, a in m/s^2.
+ * Reading R29: the bracket (the tractive power demand) is floored at 0, so a braking vehicle
+ * burns the idle rate 0.666 mL/s and never a negative amount -- the paper prints no floor, the
+ * model it cites has one.  Terms are added in the printed order. */
+float orc_fuel_rate(float v, float acc) {
+    float v2 = v * v;
+    float v3 = v2 * v;
+    float g = 0.269f * v;
+    float h = 0.0171f * v2;
+    g = g + h;
+    h = 0.000672f * v3;
+    g = g + h;
+    h = 1.680f * acc;
+    h = h * v;
+    g = g + h;
+    if (acc > 0.0f) {
+        h = acc * acc;
+        h = 0.79296f * h;
+        h = h * v;
+        g = g + h;
+    }
+    g = fmaxf(g, 0.0f);
+    float f = 0.072f * g;
+    f = 0.666f + f;
+    return f;
 }
 
 /* Fixed-time signal, one protected phase per inbound edge in round robin
@@ -284,6 +329,7 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
     S->entry_lane = xcalloc((size_t)V, 8); S->cross_node = xcalloc(V, 4);
     S->entered = xcalloc(E, 4); S->exited = xcalloc(E, 4); S->sample_count_sum = xcalloc(E, 4);
     S->exit_steps_sum = xcalloc(E, 8); S->sample_speedcode_sum = xcalloc(E, 8);
+    S->co_g = xcalloc(V, 4); S->fuel_ml = xcalloc(V, 4);
     S->n_pending = V;
     return S;
 }
@@ -303,7 +349,7 @@ void orc_destroy(orc_sim *S) {
     free(S->node_claim); free(S->touched_lanes); free(S->touched_nodes); free(S->relink);
     free(S->entry_lane); free(S->cross_node);
     free(S->entered); free(S->exited); free(S->sample_count_sum); free(S->exit_steps_sum);
-    free(S->sample_speedcode_sum);
+    free(S->sample_speedcode_sum); free(S->co_g); free(S->fuel_ml);
     free(S);
 }
 
@@ -488,6 +534,24 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
     dx = dx * p->dt;
     if (dx > cap) { dx = cap; vt = 0.0f; S->cnt.cap_bound++; }
     float xt = x + dx;
+
+    /* section 6.3.4: "since it has the position, speed, acceleration of each
+     * vehicle at every given time".  Reading R30: every step each ACTIVE vehicle adds rate * dt
+     * (the paper updates "every second"; with dt = 0.5 s this is the same integral on the
+     * simulation's own grid), with the speed v of state k and the acceleration of this step as
+     * integrated by E2, ar = (vt - v) * (1/dt), 1/dt rounded once.  A later hold at the line or
+     * a lost claim (which zero the speed) is not fed back into this step's rate. */
+    if (p->emissions) {
+        float inv_dt = 1.0f / p->dt;
+        float ar = vt - v;
+        ar = ar * inv_dt;
+        float e = orc_co_rate(v);
+        e = e * p->dt;
+        S->co_g[i] = S->co_g[i] + e;
+        float f = orc_fuel_rate(v, ar);
+        f = f * p->dt;
+        S->fuel_ml[i] = S->fuel_ml[i] + f;
+    }
 
     /* 2f */
     uint8_t act = ACT_STAY;
@@ -815,6 +879,11 @@ void orc_read_edge_stats(orc_sim *S, uint32_t *entered, uint32_t *exited,
         memset(S->exit_steps_sum, 0, E * 8); memset(S->sample_count_sum, 0, E * 4);
         memset(S->sample_speedcode_sum, 0, E * 8); S->n_samples = 0;
     }
+}
+
+void orc_read_emissions(const orc_sim *S, float *co_g, float *fuel_ml) {
+    if (co_g) memcpy(co_g, S->co_g, (size_t)S->V * 4);
+    if (fuel_ml) memcpy(fuel_ml, S->fuel_ml, (size_t)S->V * 4);
 }
 
 void orc_get_counters(const orc_sim *S, orc_counters *out) { *out = S->cnt; }

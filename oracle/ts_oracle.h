@@ -18,6 +18,13 @@
  * every neighbour by an O(V^2) search over raw (edge, lane, x) as a second, independent
  * route to the same answer.
  *
+ * Section 6.3.4 (Eq. 8 CO emission and Eq. 9 fuel consumption; SURVEY.md
+ * section 8(f) row 2) is an optional pair of per-vehicle accumulators (readings R28-R30 in
+ * DESIGN.md); it never feeds back into the traffic.  Pins: tests/test_oracle_emissions.py
+ * (values of Eq. 8 / Eq. 9 at points worked by hand from the paper's coefficients, a standing
+ * queue's idle totals, a cruising vehicle, and a fine-step fp64 quadrature of the lone-vehicle
+ * acceleration run).
+ *
  * Parity pins (tests/test_oracle_pins.py, test_oracle_invariants.py, test_oracle_scenarios.py):
  * P1 lone-vehicle closed form, P2 platoon equilibrium gap, P3 standing queue, I1-I8 invariants,
  * P4 brute force, P5 degenerate cases; scenario pins re-derived in fp64 from the rule text: the
@@ -55,6 +62,7 @@ typedef struct orc_params {
     uint32_t entry_zone_cells;
     uint32_t insert_clear_cells;
     uint32_t sample_period_steps; /* 0 = no sampling */
+    uint32_t emissions;           /* non-zero: per-vehicle CO and fuel accumulators */
 } orc_params;
 
 /* Work counters: what a byte-scan method would have to touch. */
@@ -107,6 +115,16 @@ void orc_read_state(const orc_sim *s, uint8_t *status, uint32_t *edge, uint8_t *
 void orc_read_edge_stats(orc_sim *s, uint32_t *entered, uint32_t *exited,
                          uint64_t *exit_steps_sum, uint32_t *sample_count_sum,
                          uint64_t *sample_speedcode_sum, uint32_t *n_samples, int reset);
+
+/* Per-vehicle totals since step 0, length-V arrays in vehicle-id order (PAPER.md:408-423,
+ * section 6.3.4): grams of CO (Eq. 8) and millilitres of fuel (Eq. 9).  Zeros unless
+ * orc_params.emissions was set.  Either pointer may be NULL. */
+void orc_read_emissions(const orc_sim *s, float *co_g, float *fuel_ml);
+
+/* Eq. 8 and Eq. 9 as the simulator evaluates them (fp32): CO rate in g/s at speed v (m/s);
+ * fuel rate in mL/s at speed v and acceleration acc (m/s^2). */
+float orc_co_rate(float v);
+float orc_fuel_rate(float v, float acc);
 
 void orc_get_counters(const orc_sim *s, orc_counters *out);
 void orc_destroy(orc_sim *s);
