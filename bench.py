@@ -196,6 +196,8 @@ def main():
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--sort-period", type=int, default=-1, help="steps between compaction + re-sort (tuning)")
     ap.add_argument("--profile", action="store_true", help="clock the phases inside the persistent kernel")
+    ap.add_argument("--emissions", action="store_true",
+                    help="keep the per-vehicle CO / fuel totals of PAPER.md:408-423 (SURVEY.md 8(f) row 2) during the run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end leg (profiling runs)")
     args = ap.parse_args()
@@ -224,6 +226,8 @@ def main():
         torch.cuda.synchronize()
 
     bundle = load_workload(args.workload)
+    if args.emissions:
+        bundle = dict(bundle, params=dict(bundle["params"], emissions=1))
     sim_steps = args.sim_steps or (bundle["steps"] - args.start_step)
     stream = torch.cuda.current_stream()
     sim = pkg.Sim(bundle, f"cuda:{local}", mode=args.mode)
@@ -238,6 +242,7 @@ def main():
         tuning["profile"] = 1
     for key, val in tuning.items():
         sim.set_option(key, val)
+
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")   # > 126 MB L2
 
     def one_run():
@@ -322,7 +327,7 @@ def main():
         "data": "synthetic",
         "config": {"workload": bundle["name"], "vehicles": V, "edges": bundle["n_edges"],
                    "sim_steps_per_bench_step": sim_steps, "vehicle_updates_per_bench_step": updates,
-                   "start_step": args.start_step, "tuning": tuning, "phase_ns_per_sim_step": phase_ns,
+                   "start_step": args.start_step, "tuning": tuning, "emissions": bool(args.emissions), "phase_ns_per_sim_step": phase_ns,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "step_kernel": "persistent cooperative" if args.mode == 1 else "two launches per sim step",
                    "l2": "flushed between timed iterations (256 MiB fill) and inputs (routes+atlas) exceed L2"},

@@ -96,6 +96,10 @@ typedef struct ts_params {
     uint32_t entry_zone_cells;   /* no lane change in the first cells of an edge */
     uint32_t insert_clear_cells; /* 1..16: cells of lane 0 that must be empty to insert */
     uint32_t sample_period_steps;/* PAPER.md:437 (120 = one minute); 0 = never */
+    uint32_t emissions;          /* non-zero: keep per-vehicle CO (Eq. 8) and fuel
+                                    (Eq. 9) totals; costs 8 bytes per vehicle of
+                                    workspace and one 8-byte read-modify-write per vehicle-update;
+                                    never changes the traffic (see ts_read_emissions) */
 } ts_params;
 
 /* Device resources lent by the caller for the lifetime of the ts_sim. */
@@ -159,6 +163,16 @@ int ts_reset(ts_sim *sim);
 /* Snapshot in vehicle-id order.  Synchronises; reports the sticky TS_EINVARIANT if raised. */
 int ts_read_state(ts_sim *sim, ts_state_out *out);
 int ts_read_edge_stats(ts_sim *sim, ts_edge_stats_out *out, int reset);
+
+/* Section 6.3.4 "Vehicle energy consumption and pollution estimates".
+ * Fills two caller-allocated length-V fp32 arrays in vehicle-id order (either may be NULL; HOST
+ * pointers unless ts_device.out_on_device): grams of CO emitted (Eq. 8, Stein and
+ * Walker 2003) and millilitres of fuel burnt (Eq. 9, Akcelik 1989) by each vehicle
+ * since step 0.  Every step each ACTIVE vehicle adds rate(v_k, a_k) * dt, a_k = (v_{k+1} as
+ * integrated - v_k) / dt (readings R28-R30).  Each vehicle owns its accumulators, so
+ * the fp32 sums are reproducible bit for bit.  Synchronises.  TS_EINVAL unless the sim was
+ * created with ts_params.emissions != 0. */
+int ts_read_emissions(ts_sim *sim, float *co_g, float *fuel_ml);
 
 /* Tuning knobs that never change results.
  *  "mode"          1 (default) = ts_step(n) is ONE persistent cooperative kernel looping over

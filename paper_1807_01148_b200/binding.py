@@ -16,8 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libts.so")
 TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
-           "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile", "ts_destroy",
-           "ts_last_error", "ts_version"]
+           "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile",
+           "ts_read_emissions", "ts_destroy", "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -42,7 +42,8 @@ class TsParams(C.Structure):
     _fields_ = [(n, C.c_float) for n in ("dt", "a", "b", "T", "s0", "veh_len", "b_safe", "politeness",
                                          "lc_threshold", "mand_dist_default")] + \
                [(n, C.c_uint32) for n in ("lookahead_cells", "lookback_cells", "lc_period",
-                                          "entry_zone_cells", "insert_clear_cells", "sample_period_steps")]
+                                          "entry_zone_cells", "insert_clear_cells", "sample_period_steps",
+                                          "emissions")]
 
 
 class TsDevice(C.Structure):
@@ -88,11 +89,12 @@ def load():
         L.ts_read_edge_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.ts_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
         L.ts_read_profile.argtypes = [C.c_void_p, C.c_void_p]
+        L.ts_read_emissions.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.ts_destroy.argtypes = [C.c_void_p]
         L.ts_destroy.restype = None
         L.ts_last_error.restype = C.c_char_p
         L.ts_version.restype = C.c_char_p
-        for n in EXPORTS[:9]:
+        for n in EXPORTS[:10]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -121,7 +123,8 @@ def marshal(bundle):
         "sig_green_steps", "sig_allred_steps", "sig_offset_steps")])
     routes = TsRoutes(int(b["n_vehicles"]), _p(keep["route_off"]), _p(keep["route_edges"]))
     dep = TsDepartures(_p(keep["depart_time_s"]), _p(keep["v0_mult"]), _p(keep["mand_dist_m"]))
-    prm = TsParams(**{n: b["params"][n] for n, _ in TsParams._fields_})
+    prm = TsParams(**{n: (b["params"].get(n, 0) if n == "emissions" else b["params"][n])
+                      for n, _ in TsParams._fields_})
     return net, routes, dep, prm, keep
 
 
@@ -207,6 +210,13 @@ class Sim:
                                                    "sample_count_sum", "sample_speedcode_sum")])
         _check(load().ts_read_edge_stats(self._h, C.byref(o), int(bool(reset))))
         out["n_samples"] = o.n_samples
+        return out
+
+    def read_emissions(self):
+        """Per-vehicle grams of CO (Eq. 8) and millilitres of fuel (Eq. 9)
+        since step 0; the simulation must have been created with params["emissions"] != 0."""
+        out = dict(co_g=np.zeros(self.V, np.float32), fuel_ml=np.zeros(self.V, np.float32))
+        _check(load().ts_read_emissions(self._h, _p(out["co_g"]), _p(out["fuel_ml"])))
         return out
 
     def close(self):

@@ -75,7 +75,8 @@ struct Layout {
     size_t edges, route_edges, route_begin, queue_rec, dep_rec, codes, occ, queue_state, queue_cand,
         lane_claim, node_claim, dyn, barrier, slots, mr_g, cr, rank, hist, base, audit, partial, o_status, o_lane,
         o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered, st_exited,
-        st_exit_steps, st_samp_cnt, st_samp_code, digest;
+        st_exit_steps, st_samp_cnt, st_samp_code, emis, digest;
+    uint32_t emissions = 0;
     static constexpr uint32_t kDigestChunk = 8192;
     size_t take(size_t bytes) {
         size_t off = total;
@@ -105,6 +106,7 @@ struct Layout {
         st_entered = take((size_t)E * 4); st_exited = take((size_t)E * 4);
         st_exit_steps = take((size_t)E * 8); st_samp_cnt = take((size_t)E * 4);
         st_samp_code = take((size_t)E * 8);
+        emis = take(emissions ? (size_t)V * 8 : 0);      // zeroed by ts_reset with the statistics
         digest = take((size_t)kDigestChunk * 8);
     }
 };
@@ -161,6 +163,7 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_param
     // a vehicle takes one slot when it departs; a queue head that is ready but has not won its
     // lane yet holds one reserved slot, which a compaction may drop (then it takes a new one)
     L.cap = (uint32_t)std::min<uint64_t>((uint64_t)L.V + q + 1024ull, 0x7FFFFFF0ull);
+    L.emissions = prm->emissions ? 1u : 0u;
     L.plan();
     return TS_OK;
 }
@@ -516,6 +519,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     q.H = (int)p->lookahead_cells; q.Hb = (int)p->lookback_cells;
     q.lc_pow2 = (p->lc_period && !(p->lc_period & (p->lc_period - 1))) ? 1u : 0u;
     q.lc_period = p->lc_period; q.insert_clear = p->insert_clear_cells; q.sample_period = p->sample_period_steps;
+    q.inv_dt = 1.0f / p->dt;
     c.V = L.V; c.E = L.E; c.N = L.N; c.n_queues = L.Q; c.cap_slots = L.cap; c.sort_groups = L.groups;
     c.edges = at<EdgeRec>(s, L.edges); c.route_edges = at<uint32_t>(s, L.route_edges);
     c.route_begin = at<uint32_t>(s, L.route_begin);
@@ -536,6 +540,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     c.st_entered = at<uint32_t>(s, L.st_entered); c.st_exited = at<uint32_t>(s, L.st_exited);
     c.st_exit_steps = at<unsigned long long>(s, L.st_exit_steps); c.st_samp_cnt = at<uint32_t>(s, L.st_samp_cnt);
     c.st_samp_code = at<unsigned long long>(s, L.st_samp_code);
+    c.emis = L.emissions ? at<float2>(s, L.emis) : nullptr;
 }
 
 extern "C" int ts_reset(ts_sim* s) {
@@ -829,6 +834,31 @@ extern "C" int ts_read_profile(ts_sim* s, uint64_t out[8]) {
     return TS_OK;
 }
 
+// id-ordered { CO, fuel } pairs -> two plain arrays (staged in ts_read_state's scratch)
+__global__ void k_split_emissions(const float2* __restrict__ emis, uint32_t V, float* co, float* fuel) {
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < V; i += gridDim.x * blockDim.x) {
+        const float2 e = emis[i];
+        co[i] = e.x; fuel[i] = e.y;
+    }
+}
+
+extern "C" int ts_read_emissions(ts_sim* s, float* co_g, float* fuel_ml) {
+    if (!s) return fail(TS_EINVAL, "null sim");
+    Layout& L = s->L;
+    if (!L.emissions) return fail(TS_EINVAL, "the simulation was created with ts_params.emissions == 0");
+    const size_t V = L.V;
+    if (V) {
+        k_split_emissions<<<(unsigned)std::min<size_t>(1184, (V + 255) / 256), 256, 0, s->stream>>>(
+            s->ctx.emis, L.V, at<float>(s, L.o_cell), at<float>(s, L.o_ridx));
+        CUDA_TRY(cudaGetLastError());
+    }
+    int rc = 0;
+    if ((rc = copy_out(s, co_g, s->ws + L.o_cell, V * 4))) return rc;
+    if ((rc = copy_out(s, fuel_ml, s->ws + L.o_ridx, V * 4))) return rc;
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return TS_OK;
+}
+
 extern "C" int ts_read_edge_stats(ts_sim* s, ts_edge_stats_out* o, int reset) {
     if (!s || !o) return fail(TS_EINVAL, "null argument");
     Layout& L = s->L;
@@ -844,7 +874,7 @@ extern "C" int ts_read_edge_stats(ts_sim* s, ts_edge_stats_out* o, int reset) {
     CUDA_TRY(cudaStreamSynchronize(s->stream));
     o->n_samples = d.n_samples;
     if (reset) {
-        CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, s->stream));
+        CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.emis - L.st_entered, s->stream));
         CUDA_TRY(cudaMemsetAsync(s->ws + L.dyn + offsetof(Dyn, n_samples), 0, 4, s->stream));
     }
     return TS_OK;

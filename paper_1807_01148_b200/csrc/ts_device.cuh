@@ -77,6 +77,7 @@ struct Params {
     int H, Hb;
     uint32_t lc_period, insert_clear, sample_period;
     uint32_t lc_pow2;      // lc_period is a power of two: the stagger test is a mask
+    float inv_dt;          // 1 / dt, rounded once on the host (reading R30)
 };
 // a sample is taken with the state after every sample_period-th step.
 __device__ __forceinline__ bool sample_step(const Params& p, uint32_t k) {
@@ -129,6 +130,8 @@ struct Ctx {
     // per-edge statistics
     uint32_t* st_entered; uint32_t* st_exited; unsigned long long* st_exit_steps;
     uint32_t* st_samp_cnt; unsigned long long* st_samp_code;
+    // section 6.3.4 totals, id-ordered { grams of CO, millilitres of fuel }; nullptr = not kept
+    float2* emis;
 };
 
 constexpr uint32_t kMaxCtas = 2048;
@@ -180,6 +183,26 @@ __device__ __forceinline__ float idm(const Params& p, float v, float v0, bool ha
     float q2 = q * q;
     float d = fr - q2;
     return p.a * d;
+}
+
+// Section 6.3.4.  Eq. 8: grams of CO per second at speed v; the paper's v_m is
+// in miles per hour, 1 m/s = 2.2369363 mph (reading R28).
+__device__ __forceinline__ float co_rate(float v) {
+    const float vm = v * 2.2369363f;
+    const float off = vm - 50.0f;
+    const float lin = -0.064f + 0.0056f * vm;
+    return lin + 0.00026f * (off * off);
+}
+// Eq. 9: millilitres of fuel per second at speed v (m/s) and acceleration acc (m/s^2); the engine
+// drag term only while accelerating, the power demand floored at zero (reading R29).
+__device__ __forceinline__ float fuel_rate(float v, float acc) {
+    const float v2 = v * v;
+    float dem = 0.269f * v + 0.0171f * v2;
+    dem = dem + 0.000672f * (v2 * v);
+    dem = dem + (1.680f * acc) * v;
+    if (acc > 0.0f) dem = dem + (0.79296f * (acc * acc)) * v;
+    dem = fmaxf(dem, 0.0f);
+    return 0.666f + 0.072f * dem;
 }
 
 __device__ __forceinline__ bool signal_green(const EdgeRec& e, uint32_t k) {

@@ -172,6 +172,17 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     if (dx > cap) { dx = cap; vt = 0.0f; }
     float xt = x + dx;
 
+    // section 6.3.4: this vehicle's CO and fuel totals grow by rate * dt, with
+    // the speed of state k and the acceleration just integrated (reading R30).  The vehicle owns
+    // its id-ordered pair: a plain read-modify-write, no atomics, reproducible.
+    if (c.emis) {
+        float2 em = __ldcg(c.emis + id);
+        const float ar = (vt - v) * p.inv_dt;
+        em.x = em.x + co_rate(v) * p.dt;
+        em.y = em.y + fuel_rate(v, ar) * p.dt;
+        __stcg(c.emis + id, em);
+    }
+
     // 2f + the part of step 4 that concerns nobody else: this vehicle's own state k+1
     const uint32_t gc_from = (row << 7) + (uint32_t)ci;
     const uint32_t k1 = k + 1;

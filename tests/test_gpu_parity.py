@@ -28,6 +28,10 @@ def _compare(bundle, steps, mode, chunk=None, **options):
         bad = np.nonzero(want != got)[0]
         assert bad.size == 0, f"{bundle['name']}: first digest mismatch at step {done + int(bad[0]) + 1}"
         done += n
+        if bundle["params"].get("emissions"):          # section 6.3.4 totals: fp32 bit patterns
+            ma, mb = orc.read_emissions(), sim.read_emissions()
+            for key in ("co_g", "fuel_ml"):
+                assert (ma[key].view(np.uint32) == mb[key].view(np.uint32)).all(), f"{key} after step {done}"
     a, b = orc.read_state(), sim.read_state()
     for key in ("status", "edge", "lane", "cell", "route_idx", "insert_step", "arrive_step"):
         assert (a[key] == b[key]).all(), key
