@@ -97,8 +97,8 @@ typedef struct ts_params {
     uint32_t insert_clear_cells; /* 1..16: cells of lane 0 that must be empty to insert */
     uint32_t sample_period_steps;/* PAPER.md:437 (120 = one minute); 0 = never */
     uint32_t emissions;          /* non-zero: keep per-vehicle CO (Eq. 8) and fuel
-                                    (Eq. 9) totals; costs 8 bytes per vehicle of
-                                    workspace and one 8-byte read-modify-write per vehicle-update;
+                                    (Eq. 9) totals; costs 8 bytes per vehicle plus 16 per
+                                    slot of workspace and 16 coalesced bytes per vehicle-update;
                                     never changes the traffic (see ts_read_emissions) */
 } ts_params;
 

@@ -73,7 +73,7 @@ struct Layout {
     uint32_t V = 0, E = 0, N = 0, Q = 0, cap = 0, groups = 1;
     uint64_t R = 0, n_lanes = 0, atlas_chunks = 0;   // chunk = 128 cells of one lane row
     size_t edges, route_edges, route_begin, queue_rec, dep_rec, codes, occ, queue_state, queue_cand,
-        lane_claim, node_claim, dyn, barrier, slots, mr_g, cr, rank, hist, base, audit, partial, o_status, o_lane,
+        lane_claim, node_claim, dyn, barrier, slots, slots_d, mr_g, cr, rank, hist, base, audit, partial, o_status, o_lane,
         o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered, st_exited,
         st_exit_steps, st_samp_cnt, st_samp_code, emis, digest;
     uint32_t emissions = 0;
@@ -95,6 +95,7 @@ struct Layout {
         lane_claim = take(n_lanes * 8); node_claim = take((size_t)N * 8);
         dyn = take(sizeof(Dyn)); barrier = take(256);
         slots = take((size_t)cap * 16 * 6);           // A, B, C in two ping-pong sets
+        slots_d = take(emissions ? (size_t)cap * 8 * 2 : 0);   // D in both sets
         mr_g = take((size_t)cap * 16); cr = take((size_t)cap * 32);
         rank = take((size_t)cap * 4); hist = take((size_t)E * groups * 4); base = take((size_t)E * groups * 4);
         audit = take(16);
@@ -260,7 +261,8 @@ struct PhaseClock {
 __device__ __forceinline__ void clock_tick(PhaseClock& clk, int b) { clk.tick(b); }
 
 // MAXT = most threads per SM it is launched with: sets the register budget (64 / 80 / 128).
-template <int MAXT>
+// EMIS = keep the section 6.3.4 totals (ts_params.emissions).
+template <int MAXT, bool EMIS>
 __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
                                                        uint32_t cur, uint32_t sort_period, uint32_t mr_j,
                                                        unsigned long long* digests, uint32_t profile) {
@@ -285,7 +287,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
         const uint32_t n_slots = sh_n_slots[i & 1];
         const bool sample = (k == k_sample);
         if (sample) k_sample += sp;
-        phase1(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd, qr0);
+        phase1<EMIS>(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd, qr0);
         grid_barrier(c.barrier, target, clk, 0);
         clk.tick(1);
         // slots are handed out in phase 1 only: the count the next step works on is final now
@@ -319,6 +321,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
 
 // The same phases as separate launches (mode 0: profiling per phase, and a fallback where a
 // cooperative launch is not possible).  Move records go through global memory.
+template <bool EMIS>
 __global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
     __shared__ uint32_t red[33];
     uint32_t n_upd = 0;
@@ -327,7 +330,7 @@ __global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, u
     __syncthreads();
     const uint32_t n_slots = sh_n;
     const Who me = who();
-    phase1(c, c.s[cur], k, me, nullptr, 0, n_slots, sample_step(c.p, k), n_upd, first_queue_rec(c, me));
+    phase1<EMIS>(c, c.s[cur], k, me, nullptr, 0, n_slots, sample_step(c.p, k), n_upd, first_queue_rec(c, me));
     if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n_slots;   // phase 2 overwrites dyn->n_slots
     n_upd = block_sum(n_upd, red);
     if (threadIdx.x == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
@@ -434,12 +437,16 @@ __global__ void k_finish_state(const __grid_constant__ Ctx c, uint32_t* o_cell, 
 
 // The instantiation whose register budget fits `per_sm_threads` resident threads per SM
 // (128 / 96 / 80 / 72 / 64 registers per thread).
-static const void* step_kernel(int per_sm_threads) {
-    if (per_sm_threads <= 512) return (const void*)k_persistent<512>;
-    if (per_sm_threads <= 640) return (const void*)k_persistent<640>;
-    if (per_sm_threads <= 768) return (const void*)k_persistent<768>;
-    if (per_sm_threads <= 896) return (const void*)k_persistent<896>;
-    return (const void*)k_persistent<1024>;
+template <bool EMIS>
+static const void* step_kernel_of(int per_sm_threads) {
+    if (per_sm_threads <= 512) return (const void*)k_persistent<512, EMIS>;
+    if (per_sm_threads <= 640) return (const void*)k_persistent<640, EMIS>;
+    if (per_sm_threads <= 768) return (const void*)k_persistent<768, EMIS>;
+    if (per_sm_threads <= 896) return (const void*)k_persistent<896, EMIS>;
+    return (const void*)k_persistent<1024, EMIS>;
+}
+static const void* step_kernel(int per_sm_threads, bool emissions) {
+    return emissions ? step_kernel_of<true>(per_sm_threads) : step_kernel_of<false>(per_sm_threads);
 }
 
 // ------------------------------------------------------------------ create / reset
@@ -531,6 +538,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     uint4* sl = at<uint4>(s, L.slots);
     const size_t cap = L.cap;
     for (int i = 0; i < 2; i++) { c.s[i].A = sl + (3 * i + 0) * cap; c.s[i].B = sl + (3 * i + 1) * cap; c.s[i].C = sl + (3 * i + 2) * cap; }
+    for (int i = 0; i < 2; i++) c.s[i].D = L.emissions ? at<float2>(s, L.slots_d) + i * cap : nullptr;
     c.mr_g = at<uint4>(s, L.mr_g); c.cr = at<uint4>(s, L.cr);
     c.rank = at<uint32_t>(s, L.rank); c.hist = at<uint32_t>(s, L.hist); c.base = at<uint32_t>(s, L.base);
     c.partial = at<uint32_t>(s, L.partial); c.audit = at<unsigned long long>(s, L.audit);
@@ -665,7 +673,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     cudaDeviceGetAttribute(&s->smem_limit, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_id);
     bool attr_ok = true;
     for (int t : {512, 640, 768, 896, 1024})
-        attr_ok = attr_ok && cudaFuncSetAttribute(step_kernel(t), cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) == cudaSuccess;
+        attr_ok = attr_ok && cudaFuncSetAttribute(step_kernel(t, s->L.emissions != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) == cudaSuccess;
     if (!attr_ok) {
         delete s;
         return fail(TS_ECUDA, "cannot raise the dynamic shared memory limit of the step kernel");
@@ -718,7 +726,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
         mr_j = std::min(mr_j, need_j);
         const size_t smem = (size_t)mr_j * 16 * s->threads;
         const int per_sm_threads = s->threads * s->blocks_per_sm;
-        const void* kern = step_kernel(per_sm_threads);
+        const void* kern = step_kernel(per_sm_threads, s->L.emissions != 0);
         int per_sm = 0;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, s->threads, smem));
         if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, s->threads);
@@ -731,7 +739,8 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
         const int g = s->sms * 8, gs = std::min<int>(s->sms * 8, (int)kMaxCtas);
         for (uint32_t i = 0; i < n; i++) {
             const uint32_t k = s->k + i;
-            k_phase1<<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            if (s->L.emissions) k_phase1<true><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            else k_phase1<false><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
             k_phase2<<<g, 256, 0, st>>>(s->ctx, k, s->cur);
             if (d_digests) k_digest<<<g, 256, 0, st>>>(s->ctx, s->cur, d_digests + i);
             if (R && (k + 1) % R == 0) {
@@ -834,6 +843,15 @@ extern "C" int ts_read_profile(ts_sim* s, uint64_t out[8]) {
     return TS_OK;
 }
 
+// totals of the vehicles still driving: slot-ordered -> id-ordered (arrived ones are there already)
+__global__ void k_gather_emissions(const __grid_constant__ Ctx c, uint32_t cur) {
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+    const uint32_t n_slots = min(c.dyn->slot_alloc, c.cap_slots);
+    const Slots& S = c.s[cur];
+    for (uint32_t s = tid; s < n_slots; s += nthreads)
+        if (S.A[s].w & ALIVE) c.emis[S.B[s].z] = S.D[s];
+}
+
 // id-ordered { CO, fuel } pairs -> two plain arrays (staged in ts_read_state's scratch)
 __global__ void k_split_emissions(const float2* __restrict__ emis, uint32_t V, float* co, float* fuel) {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < V; i += gridDim.x * blockDim.x) {
@@ -848,6 +866,7 @@ extern "C" int ts_read_emissions(ts_sim* s, float* co_g, float* fuel_ml) {
     if (!L.emissions) return fail(TS_EINVAL, "the simulation was created with ts_params.emissions == 0");
     const size_t V = L.V;
     if (V) {
+        k_gather_emissions<<<1184, 256, 0, s->stream>>>(s->ctx, s->cur);
         k_split_emissions<<<(unsigned)std::min<size_t>(1184, (V + 255) / 256), 256, 0, s->stream>>>(
             s->ctx.emis, L.V, at<float>(s, L.o_cell), at<float>(s, L.o_ridx));
         CUDA_TRY(cudaGetLastError());

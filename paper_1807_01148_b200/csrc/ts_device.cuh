@@ -89,10 +89,12 @@ __device__ __forceinline__ bool sample_step(const Params& p, uint32_t k) {
 //   A = { bits(x), bits(v), row (first chunk of the vehicle's lane row), lane | ALIVE }
 //   B = { edge, next route edge or NONE32, vehicle id, bits(v0_mult) }
 //   C = { route position, one past the last route position, step it entered the edge, bits(mand_dist) }
+//   D = { grams of CO, millilitres of fuel } so far (section 6.3.4; nullptr when not kept)
 struct Slots {
     uint4* A;
     uint4* B;
     uint4* C;
+    float2* D;
 };
 
 // Everything the kernels touch.  Passed by value.
@@ -130,7 +132,8 @@ struct Ctx {
     // per-edge statistics
     uint32_t* st_entered; uint32_t* st_exited; unsigned long long* st_exit_steps;
     uint32_t* st_samp_cnt; unsigned long long* st_samp_code;
-    // section 6.3.4 totals, id-ordered { grams of CO, millilitres of fuel }; nullptr = not kept
+    // section 6.3.4 totals, id-ordered { grams of CO, millilitres of fuel }: written when a vehicle
+    // arrives and by ts_read_emissions' gather (while it drives they live in Slots::D); nullptr = not kept
     float2* emis;
 };
 

@@ -18,12 +18,16 @@ namespace ts {
 
 // DESIGN.md 2, steps 2a-2f for one slot.  Reads state k and atlas M_k only; returns the move
 // record that phase 2 applies.  `n_upd` counts ACTIVE vehicles advanced (the metric's unit).
+// EMIS: keep the section 6.3.4 totals (compiled out of the default instantiation).
+template <bool EMIS>
 __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, uint32_t slot, uint32_t k,
                                                 bool sample, uint32_t& n_upd) {
     const Params& p = c.p;
     // trip 1: slot state
     const uint4 sa = ldcg4(S.A + slot);
     const uint4 sb = ldcg4(S.B + slot);
+    float2 em = make_float2(0.0f, 0.0f);               // section 6.3.4 totals so far (slot-ordered: coalesced)
+    if (EMIS) em = __ldcg(S.D + slot);
     if (!(sa.w & ALIVE)) return make_uint4(0, 0, 0, MR_NONE);
     n_upd++;
     const float x = __uint_as_float(sa.x), v = __uint_as_float(sa.y);
@@ -173,14 +177,13 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     float xt = x + dx;
 
     // section 6.3.4: this vehicle's CO and fuel totals grow by rate * dt, with
-    // the speed of state k and the acceleration just integrated (reading R30).  The vehicle owns
-    // its id-ordered pair: a plain read-modify-write, no atomics, reproducible.
-    if (c.emis) {
-        float2 em = __ldcg(c.emis + id);
+    // the speed of state k and the acceleration just integrated (reading R30).  The pair travels
+    // with the vehicle's slot: a plain read-modify-write, no atomics, reproducible.
+    if (EMIS) {
         const float ar = (vt - v) * p.inv_dt;
         em.x = em.x + co_rate(v) * p.dt;
         em.y = em.y + fuel_rate(v, ar) * p.dt;
-        __stcg(c.emis + id, em);
+        __stcg(S.D + slot, em);
     }
 
     // 2f + the part of step 4 that concerns nobody else: this vehicle's own state k+1
@@ -192,6 +195,7 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
             stcg4(S.A + slot, make_uint4(__float_as_uint(Cf), __float_as_uint(vt), row, l));
             c.o_status[id] = 2; c.o_arrive[id] = k1; c.o_x[id] = Cf; c.o_v[id] = vt;
             c.o_edge[id] = e; c.o_lane[id] = (uint8_t)l; c.o_rpos[id] = sc.x;
+            if (EMIS) c.emis[id] = em;                 // final totals, id-ordered
             atomicAdd(c.st_exited + e, 1u);
             atomicAdd(c.st_exit_steps + e, (unsigned long long)(k1 - sc.z));
             atomicAdd(&c.dyn->n_arrived, 1u);
@@ -248,6 +252,7 @@ __device__ __forceinline__ void departure_phase1(const Ctx& c, const Slots& S, u
                 stcg4(S.A + slot, make_uint4(0u, 0u, qr.x, 0u));                    // x = 0, v = 0, lane 0, not alive
                 stcg4(S.B + slot, make_uint4(qr.w, d1.y, d0.x, d0.y));
                 stcg4(S.C + slot, make_uint4(d0.w, d1.x, k + 1, d0.z));
+                if (S.D) __stcg(S.D + slot, make_float2(0.0f, 0.0f));
                 atomicMin(c.lane_claim + qr.y, claim_word(k, d0.x));
                 cand = make_uint4(d0.x, slot, qs.x, dep_next);
             }
@@ -330,12 +335,13 @@ __device__ __forceinline__ void departure_phase2(const Ctx& c, const Slots& S, u
 
 // `n_slots` must reach the threads without every warp of the grid loading the same word (one
 // L2 slice would serve ~5000 requests in turn): one thread per CTA reads it, see the kernels.
+template <bool EMIS>
 __device__ __forceinline__ void phase1(const Ctx& c, const Slots& S, uint32_t k, const Who& me, uint4* mr_s,
                                        uint32_t mr_j, uint32_t n_slots, bool sample, uint32_t& n_upd, const uint4 qr0) {
     for (uint32_t j = 0;; j++) {
         const uint32_t s = me.slot(j);
         if (s >= n_slots) break;
-        const uint4 mr = vehicle_phase1(c, S, s, k, sample, n_upd);
+        const uint4 mr = vehicle_phase1<EMIS>(c, S, s, k, sample, n_upd);
         if (j < mr_j) mr_s[j * me.T + me.t] = mr; else stcg4(c.mr_g + s, mr);
     }
     for (uint32_t j = 0;; j++) {

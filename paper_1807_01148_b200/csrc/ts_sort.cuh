@@ -118,6 +118,7 @@ __device__ __forceinline__ void sort_scatter(const Ctx& c, const Slots& from, co
         const uint4 sa = ldcg4(from.A + s), sb = ldcg4(from.B + s), sc = ldcg4(from.C + s);
         const uint32_t d = __ldcg(c.base + sort_key(c, sb)) + r;
         stcg4(to.A + d, sa); stcg4(to.B + d, sb); stcg4(to.C + d, sc);
+        if (from.D) __stcg(to.D + d, __ldcg(from.D + s));
     }
 }
 

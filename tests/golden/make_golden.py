@@ -3,6 +3,7 @@
 workload of a BASELINE.json config, full length.
 
     python tests/golden/make_golden.py cfg1 cfg2 cfg3 cfg5 [--stride 600]
+    python tests/golden/make_golden.py --emissions cfg1 cfg2 cfg5      # writes emissions_<cfg>.json
 
 Stored per config (nothing here ever comes from the CUDA path):
   sha256     checksum of the generated input bundle (detects generator drift between machines)
@@ -17,6 +18,9 @@ Stored per config (nothing here ever comes from the CUDA path):
   edge_stats sums of the oracle's per-edge accumulators at the last mark (entered, exited,
              exit_steps_sum, sample_count_sum, sample_speedcode_sum, n_samples) and a position-weighted
              checksum of each: the digests do not cover these
+  (--emissions: a separate file emissions_<cfg>.json with the whole-run totals of the section
+             6.3.4 accumulators: per array the fp64 sum, the sum of the fp32 bit
+             patterns and a position-weighted sum of the bit patterns, plus the final digest)
   complete   false while the run is in progress: the file is rewritten after every stride, so an
              interrupted run of a very long config (config 4: 5.4e10 vehicle-updates, many hours of
              the single-threaded oracle) still leaves a usable prefix of digests
@@ -71,11 +75,44 @@ def run(name, stride, suffix=""):
     print(name, "->", path, f"{out['seconds']:.0f} s", out["counters"]["updates"], "updates", flush=True)
 
 
+def _bits_checksums(a):
+    u = np.asarray(a, np.float32).view(np.uint32).astype(np.uint64)
+    w = np.arange(1, len(u) + 1, dtype=np.uint64)
+    return dict(sum=float(np.asarray(a, np.float64).sum()), bits_sum=int(u.sum()),
+                bits_weighted=int((u * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF)))
+
+
+def run_emissions(name, stride):
+    bundle = W.by_name(name)
+    sha = W.bundle_sha256(bundle)
+    bundle = dict(bundle, params=dict(bundle["params"], emissions=1))
+    orc = Oracle(bundle)
+    steps = bundle["steps"]
+    t0 = time.perf_counter()
+    done, last = 0, None
+    while done < steps:
+        n = min(stride, steps - done)
+        last = orc.step(n, digests=True)[-1]
+        done += n
+    em = orc.read_emissions()
+    out = dict(name=bundle["name"], sha256=sha, steps=steps, final_digest=f"{int(last):016x}",
+               updates=orc.counters()["updates"], co_g=_bits_checksums(em["co_g"]),
+               fuel_ml=_bits_checksums(em["fuel_ml"]), seconds=round(time.perf_counter() - t0, 1))
+    path = os.path.join(HERE, f"emissions_{name}.json")
+    with open(path, "w") as f:
+        json.dump(out, f, indent=1)
+    print(name, "->", path, f"{out['seconds']:.0f} s", flush=True)
+
+
 if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("configs", nargs="+")
     ap.add_argument("--stride", type=int, default=600)
     ap.add_argument("--suffix", default="", help="write trace_<cfg><suffix>.json (a second, incremental run beside a long one)")
+    ap.add_argument("--emissions", action="store_true", help="write emissions_<cfg>.json instead of a trace")
     a = ap.parse_args()
     for c in a.configs:
-        run(c, a.stride, a.suffix)
+        if a.emissions:
+            run_emissions(c, a.stride)
+        else:
+            run(c, a.stride, a.suffix)

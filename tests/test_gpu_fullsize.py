@@ -63,3 +63,30 @@ def test_full_run_matches_golden_digests(name):
             assert int((v * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF)) == weighted, key
     assert np.all(np.diff(tr["marks"]) > 0)
     sim.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5"])
+def test_full_run_emission_totals(name):
+    """Section 6.3.4 at full size, default launch configuration, WHOLE run: the
+    oracle's per-vehicle CO and fuel totals are stored as checksums of their fp32 bit patterns
+    (tests/golden/emissions_<cfg>.json, written by make_golden.py --emissions from oracle/ only)."""
+    import paper_1807_01148_b200 as pkg
+    from paper_1807_01148_b200 import workload as W
+    path = os.path.join(GOLDEN, f"emissions_{name}.json")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated yet (tests/golden/make_golden.py --emissions {name})")
+    tr = json.load(open(path))
+    b = W.by_name(name)
+    assert W.bundle_sha256(b) == tr["sha256"]
+    sim = pkg.Sim(dict(b, params=dict(b["params"], emissions=1)), "cuda:0")
+    sim.step(tr["steps"] - 1)
+    assert f"{int(sim.step_digest(1)[0]):016x}" == tr["final_digest"]
+    assert sim.read_counts()["vehicle_updates"] == tr["updates"]
+    em = sim.read_emissions()
+    for key in ("co_g", "fuel_ml"):
+        u = em[key].view(np.uint32).astype(np.uint64)
+        w = np.arange(1, len(u) + 1, dtype=np.uint64)
+        assert int(u.sum()) == tr[key]["bits_sum"], key
+        assert int((u * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF)) == tr[key]["bits_weighted"], key
+        assert float(em[key].astype(np.float64).sum()) == tr[key]["sum"], key
+    sim.close()
