@@ -39,7 +39,7 @@ enum : uint32_t { MR_NONE = 0, MR_MOVE = 1, MR_CLEAR = 2, MR_CROSS = 3 };
 
 // 32 bytes per edge: everything a vehicle needs to know about the edge it is on (or enters),
 // including the signal plan of the node at its head, in two 16-byte loads.
-struct __align__(16) EdgeRec {
+struct __align__(32) EdgeRec {
     uint32_t row;        // atlas offset of lane 0's row, in chunks of 128 cells
     uint32_t lane_base;  // global lane index of lane 0 (index of its claim word)
     float vlim;          // m/s
@@ -215,12 +215,14 @@ __device__ __forceinline__ bool signal_green(const EdgeRec& e, uint32_t k) {
     return t - (uint32_t)e.in_rank * e.P < e.green;       // unsigned: t below the phase start wraps
 }
 
+// One 256-bit load (sm_100 LDG.256): a record is one 32-byte sector, and a warp whose vehicles sit
+// on 20 different edges pays for 20 sectors once instead of twice.
 __device__ __forceinline__ EdgeRec load_edge(const EdgeRec* edges, uint32_t e) {
-    const uint4* p = reinterpret_cast<const uint4*>(edges + e);
-    uint4 a = __ldg(p), b = __ldg(p + 1);
     EdgeRec r;
-    uint4* q = reinterpret_cast<uint4*>(&r);
-    q[0] = a; q[1] = b;
+    uint32_t* w = reinterpret_cast<uint32_t*>(&r);
+    asm("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]), "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7])
+        : "l"(edges + e));
     return r;
 }
 __device__ __forceinline__ uint32_t edge_lanes(const EdgeRec& e) { return e.lanes_ctrl & 15u; }
