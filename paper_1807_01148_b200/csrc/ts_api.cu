@@ -239,7 +239,7 @@ extern __shared__ uint4 dyn_smem[];
 
 // The static record of the first (normally the only) departure queue this thread looks after.
 __device__ __forceinline__ uint4 first_queue_rec(const Ctx& c, const Who& me) {
-    const uint32_t q = me.slot(0);
+    const uint32_t q = me.qslot(0);
     return q < c.n_queues ? __ldg(c.queue_rec + q) : make_uint4(0, 0, 0, 0);
 }
 

@@ -149,6 +149,13 @@ struct Who {
     __device__ __forceinline__ uint32_t slot(uint32_t j) const {
         return ((j * (T >> 5) + (t >> 5)) * n_cta + cta) * 32u + (t & 31u);
     }
+    // Departure queues are dealt the same way but to the warps of a CTA in REVERSE order: the first
+    // warps are the ones that get one more tile of vehicles whenever the tiles do not divide evenly,
+    // so the queue heads (an L2 round trip of their own in each phase) go to the warps with slack.
+    __device__ __forceinline__ uint32_t qslot(uint32_t j) const {
+        const uint32_t W = T >> 5;
+        return ((j * W + (W - 1u - (t >> 5))) * n_cta + cta) * 32u + (t & 31u);
+    }
     __device__ __forceinline__ uint32_t gtid() const { return cta * T + t; }
     __device__ __forceinline__ uint32_t gthreads() const { return n_cta * T; }
 };

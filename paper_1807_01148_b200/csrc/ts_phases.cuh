@@ -345,7 +345,7 @@ __device__ __forceinline__ void phase1(const Ctx& c, const Slots& S, uint32_t k,
         if (j < mr_j) mr_s[j * me.T + me.t] = mr; else stcg4(c.mr_g + s, mr);
     }
     for (uint32_t j = 0;; j++) {
-        const uint32_t q = me.slot(j);
+        const uint32_t q = me.qslot(j);
         if (q - (q & 31u) >= c.n_queues) break;
         if (q < c.n_queues) departure_phase1(c, S, q, k, j == 0 ? qr0 : __ldg(c.queue_rec + q));
     }
@@ -366,7 +366,7 @@ __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k,
         vehicle_phase2(c, S, s, k, sample, mr);
     }
     for (uint32_t j = 0;; j++) {
-        const uint32_t q = me.slot(j);
+        const uint32_t q = me.qslot(j);
         if (q - (q & 31u) >= c.n_queues) break;
         if (q < c.n_queues) departure_phase2(c, S, q, k, sample, j == 0 ? qr0 : __ldg(c.queue_rec + q));
     }
