@@ -38,6 +38,17 @@ def test_query_workspace_and_validation_without_gpu(cfg1):
     assert ei.value.code == binding.TS_EINVAL and "length" in str(ei.value)
 
 
+def test_emission_totals_are_paid_for_only_when_asked(cfg1):
+    """ts_params.emissions adds 8 bytes per vehicle and 16 per slot to the
+    workspace; without it the layout is the one it was."""
+    from paper_1807_01148_b200 import binding
+    plain = binding.query_workspace(cfg1)
+    with_totals = binding.query_workspace(dict(cfg1, params=dict(cfg1["params"], emissions=1)))
+    V, E = cfg1["n_vehicles"], cfg1["n_edges"]
+    slots = V + E + 1024                       # upper bound of the slot capacity (vehicles + queues + slack)
+    assert plain + 8 * V + 16 * V <= with_totals <= plain + 8 * V + 16 * slots + 512
+
+
 def test_no_cpu_fallback(cfg1):
     """Without a CUDA device ts_create must fail loudly, not fall back."""
     import torch
