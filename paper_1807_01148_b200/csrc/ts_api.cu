@@ -586,6 +586,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     // per-edge records: atlas row offsets, claim indices, signal plan of the head node
     std::vector<uint32_t> n_in(N, 0);
     std::vector<EdgeRec> edges(E);
+    std::vector<uint8_t> in_rank(E);
     uint64_t row = 0, lane_base = 0;
     for (uint32_t e = 0; e < E; e++) {
         EdgeRec& r = edges[e];
@@ -593,22 +594,32 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         if (n_in[h] >= 255) return fail(TS_EINVAL, "node %u: more than 255 inbound edges", h);
         r.row = (uint32_t)row; r.lane_base = (uint32_t)lane_base; r.vlim = net->edge_vlim[e];
         r.to_node = h; r.len = (uint16_t)net->edge_len_m[e];
-        r.lanes_ctrl = (uint8_t)(net->edge_lanes[e] | (ctrl << 4));
-        r.in_rank = (uint8_t)n_in[h]++;
-        r.green = 1; r.P = 1; r.cycle = 1; r.offset = 0;
-        if (ctrl == TS_CTRL_SIGNAL) {
-            r.green = (uint16_t)net->sig_green_steps[h];
-            r.P = (uint16_t)(net->sig_green_steps[h] + net->sig_allred_steps[h]);
-            r.offset = net->sig_offset_steps[h];
-        }
+        r.cyc_lc = 1u | ((uint32_t)net->edge_lanes[e] << 24) | (ctrl << 28);
+        r.off_sh = 0; r.magic = 1; r.green = 1;          // cycle 1: n mod 1 = 0 < green
+        in_rank[e] = (uint8_t)n_in[h]++;
         row += (uint64_t)net->edge_lanes[e] * ((net->edge_len_m[e] + 127) >> 7);
         lane_base += net->edge_lanes[e];
     }
-    for (uint32_t e = 0; e < E; e++)
-        if ((edges[e].lanes_ctrl >> 4) == TS_CTRL_SIGNAL) {
-            uint64_t cyc = (uint64_t)n_in[edges[e].to_node] * edges[e].P;
-            edges[e].cycle = (uint32_t)cyc;
-        }
+    // A1 (reading R16): inbound edge number in_rank of node h is green at step k iff
+    // t = (k + offset_h) mod (n_in * P) lies in [in_rank * P, in_rank * P + green), P = green + allred.
+    // Shifting the offset by the phase start turns that into one comparison, and the modulo by the
+    // invariant cycle is done by multiplication on the device (ts_device.cuh).
+    for (uint32_t e = 0; e < E; e++) {
+        EdgeRec& r = edges[e];
+        if ((r.cyc_lc >> 28) != TS_CTRL_SIGNAL) continue;
+        const uint32_t h = r.to_node;
+        const uint64_t P = (uint64_t)net->sig_green_steps[h] + net->sig_allred_steps[h];
+        const uint64_t cycle = (uint64_t)n_in[h] * P;                    // <= 255 * 65535 < 2^24
+        const uint64_t start = (uint64_t)in_rank[e] * P;                 // < cycle
+        const uint64_t off = ((uint64_t)net->sig_offset_steps[h] % cycle + cycle - start) % cycle;
+        uint32_t l = 0;
+        while ((1ull << l) < cycle) l++;
+        const uint32_t sh1 = l ? 1u : 0u, sh2 = l - sh1;
+        r.magic = (uint32_t)(((1ull << 32) * ((1ull << l) - cycle)) / cycle + 1ull);
+        r.cyc_lc = (uint32_t)cycle | (r.cyc_lc & 0xFF000000u);
+        r.off_sh = (uint32_t)off | (sh1 << 24) | (sh2 << 25);
+        r.green = (uint16_t)net->sig_green_steps[h];
+    }
     // departure queues: per first edge, FIFO by (departure step, id) (R19)
     std::vector<uint32_t> dep_step(V), route_begin(V), order(V);
     for (uint32_t i = 0; i < V; i++) {

@@ -44,12 +44,15 @@ struct __align__(32) EdgeRec {
     uint32_t lane_base;  // global lane index of lane 0 (index of its claim word)
     float vlim;          // m/s
     uint32_t to_node;
-    uint32_t cycle;      // n_in * (green + allred) at a SIGNAL head node, else 1
-    uint32_t offset;     // signal offset, steps
-    uint16_t green, P;   // P = green + allred
+    // Signal plan of the head node, reduced on the host to "green iff (k + off) mod cycle < green"
+    // (off = offset - in_rank * (green + allred), mod cycle), with the modulo by the run-time
+    // invariant `cycle` done by multiplication (Granlund & Montgomery 1994, N = 32):
+    //   t = mulhi(magic, n);  q = (t + ((n - t) >> sh1)) >> sh2;  n mod cycle = n - q * cycle.
+    uint32_t cyc_lc;     // cycle (n_in * (green + allred), < 2^24; 1 where not SIGNAL) | lanes << 24 | ctrl << 28
+    uint32_t off_sh;     // off (< cycle) | sh1 << 24 | sh2 << 25
+    uint32_t magic;      // floor(2^32 (2^l - cycle) / cycle) + 1, l = ceil(log2 cycle)
+    uint16_t green;      // steps
     uint16_t len;        // cells
-    uint8_t lanes_ctrl;  // lanes | ctrl << 4
-    uint8_t in_rank;     // rank among the inbound edges of the head node
 };
 static_assert(sizeof(EdgeRec) == 32, "EdgeRec must be 32 bytes");
 
@@ -216,10 +219,11 @@ __device__ __forceinline__ float fuel_rate(float v, float acc) {
 }
 
 __device__ __forceinline__ bool signal_green(const EdgeRec& e, uint32_t k) {
-    // green iff t div P == in_rank and t mod P < green, i.e. in_rank * P <= t < in_rank * P + green:
-    // one modulo, no division
-    const uint32_t t = (k + e.offset) % e.cycle;          // k, offset < 2^31
-    return t - (uint32_t)e.in_rank * e.P < e.green;       // unsigned: t below the phase start wraps
+    const uint32_t cycle = e.cyc_lc & 0xFFFFFFu;
+    const uint32_t n = k + (e.off_sh & 0xFFFFFFu);        // k < 2^31, off < 2^24
+    const uint32_t t = __umulhi(e.magic, n);
+    const uint32_t q = (t + ((n - t) >> ((e.off_sh >> 24) & 1u))) >> (e.off_sh >> 25);
+    return n - q * cycle < (uint32_t)e.green;
 }
 
 // One 256-bit load (sm_100 LDG.256): a record is one 32-byte sector, and a warp whose vehicles sit
@@ -232,8 +236,8 @@ __device__ __forceinline__ EdgeRec load_edge(const EdgeRec* edges, uint32_t e) {
         : "l"(edges + e));
     return r;
 }
-__device__ __forceinline__ uint32_t edge_lanes(const EdgeRec& e) { return e.lanes_ctrl & 15u; }
-__device__ __forceinline__ uint32_t edge_ctrl(const EdgeRec& e) { return e.lanes_ctrl >> 4; }
+__device__ __forceinline__ uint32_t edge_lanes(const EdgeRec& e) { return (e.cyc_lc >> 24) & 15u; }
+__device__ __forceinline__ uint32_t edge_ctrl(const EdgeRec& e) { return e.cyc_lc >> 28; }
 __device__ __forceinline__ uint32_t row_stride(const EdgeRec& e) { return ((uint32_t)e.len + 127u) >> 7; }
 __device__ __forceinline__ uint32_t lane_row(const EdgeRec& e, uint32_t lane) { return e.row + lane * row_stride(e); }
 

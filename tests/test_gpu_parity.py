@@ -185,3 +185,27 @@ def test_chunking_across_sort_boundaries():
         st = sim.read_state()
         assert st["step"] == 600
         sim.close()
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_signal_plans_of_every_shape(seed):
+    """A1: the device reduces the signal test to one comparison after a modulo by multiplication.
+    Plans that stress it: green of one step with no all-red (cycle = in-degree, down to 1),
+    power-of-two and odd cycles, phases up to 65 535 steps, offsets up to 2^31 - 1."""
+    rng = np.random.default_rng(seed)
+    b = small_signal_grid(seed=seed, n_vehicles=900, steps=1200)
+    N = b["n_nodes"]
+    green = rng.choice([1, 2, 3, 7, 8, 16, 31, 64, 100, 257, 4096, 65535], N)
+    allred = rng.choice([0, 0, 1, 2, 5, 8, 60], N)
+    allred = np.where(green + allred > 65535, 0, allred)
+    offset = rng.choice([0, 1, 5, 1000, 2 ** 24 + 3, 2 ** 31 - 1, 2 ** 31 - 2, 123456789], N)
+    b = dict(b, sig_green_steps=green.astype(np.uint32), sig_allred_steps=allred.astype(np.uint32),
+             sig_offset_steps=offset.astype(np.uint32))
+    _compare(b, 1200, 1, chunk=400)
+    _compare(b, 300, 0)
+    if seed == 11:                             # one inbound edge, green 1 + all-red 0: cycle 1, always green
+        n = 3
+        one = (np.full(n, 1), np.full(n, 0), np.full(n, 2 ** 31 - 1))
+        _compare(corridor(n_edges=2, length=300, departs=np.arange(8) * 3.0, ctrl=2, sig=one), 600, 1)
+        two = (np.full(n, 1), np.full(n, 1), np.full(n, 7))            # cycle 2: green on alternate steps
+        _compare(corridor(n_edges=2, length=300, departs=np.arange(8) * 3.0, ctrl=2, sig=two), 600, 1)
