@@ -320,6 +320,11 @@ def main():
     bpu, cells, bsrc = bytes_per_update(args.workload)
     launch_s = (sum(ms) / len(ms)) / 1e3                  # one k_persistent launch per bench step
     achieved = bpu * updates / launch_s / 1e9
+    # mode 1: one cooperative launch per ts_step call, or -- adaptive CTA size, the default when no
+    # geometry is asked for -- two per chunk of 2048 steps, of which the device runs one
+    adaptive = args.mode == 1 and not (args.threads or args.blocks_per_sm or args.profile)
+    launches_per_run = (2 * sim_steps if args.mode != 1 else
+                        2 * ((sim_steps + 2047) // 2048) if adaptive else 1)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
@@ -329,11 +334,12 @@ def main():
                    "sim_steps_per_bench_step": sim_steps, "vehicle_updates_per_bench_step": updates,
                    "start_step": args.start_step, "tuning": tuning, "emissions": bool(args.emissions), "phase_ns_per_sim_step": phase_ns,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "step_kernel": "persistent cooperative" if args.mode == 1 else "two launches per sim step",
+                   "step_kernel": ("persistent cooperative, CTA size chosen on the device per 2048 steps (640 / 896 threads)" if adaptive
+                                   else "persistent cooperative" if args.mode == 1 else "two launches per sim step"),
                    "l2": "flushed between timed iterations (256 MiB fill) and inputs (routes+atlas) exceed L2"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": sum(e2e_ms) / len(e2e_ms) if e2e_ms else None},
-        "gpu_launches": args.steps * (1 if args.mode == 1 else 2 * sim_steps),
+        "gpu_launches": args.steps * launches_per_run,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak,

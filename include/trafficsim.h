@@ -177,7 +177,14 @@ int ts_read_emissions(ts_sim *sim, float *co_g, float *fuel_ml);
 /* Tuning knobs that never change results.
  *  "mode"          1 (default) = ts_step(n) is ONE persistent cooperative kernel looping over
  *                  the n steps with grid-wide barriers; 0 = one launch per phase.
- *  "threads"       CTA size of the persistent kernel (multiple of 32 in 64..1024, default 640).
+ *  "threads"       CTA size of the persistent kernel (multiple of 32 in 64..1024).  Default: not
+ *                  fixed -- ts_step enqueues every chunk of 2048 steps twice, with 640 threads
+ *                  (spill-free; best while a step is one warp's latency) and with 896 (more warps;
+ *                  best once a CTA holds several rounds of vehicles), and the device runs the one
+ *                  that fits the number of live slots; the other launch returns at once.  Setting
+ *                  "threads" or "blocks_per_sm" (or "profile") fixes the size; "adaptive" 1 undoes it.
+ *  "adaptive_chunk", "adaptive_above"  steps per chunk (default 2048) and the number of live slots
+ *                  above which the 896-thread size is preferred (default 640 per SM; -1 restores it).
  *  "blocks_per_sm" resident CTAs per SM of the persistent kernel (default 1).
  *  "sort_period"   steps between compaction of retired slots + re-sort of the live ones by
  *                  edge; 0 = never; default 128 (256 on networks

@@ -193,10 +193,15 @@ struct ts_sim {
     int mode = 1;             // 0: one launch per phase, 1: persistent cooperative kernel
     int threads = 640;        // persistent kernel CTA size (96 registers per thread, no spills: within 4 % of the best size for 3e4 and for 3e5 active vehicles)
     int blocks_per_sm = 1;
+    uint32_t chunk_no = 0;    // adaptive chunks enqueued since ts_reset (parity selects Dyn::prefer_big[])
+    uint32_t adaptive_chunk = 2048;   // steps per adaptive chunk
+    long long adaptive_above = -1;    // live slots above which the big CTA size is preferred (-1: one round of tiles at 640 threads)
+    int adaptive = 1;         // no CTA size asked for: 640 threads, or 896 while more than one round of tiles is live
     int sms = 0;
     uint32_t sort_period = 128;  // steps between compaction + re-sort; 0 = never (set in ts_create)
     uint32_t profile = 0;
     int smem_limit = 0;
+    int l2_bytes = 0;
     uint32_t sticky = 0;
 };
 
@@ -265,11 +270,21 @@ __device__ __forceinline__ void clock_tick(PhaseClock& clk, int b) { clk.tick(b)
 template <int MAXT, bool EMIS>
 __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
                                                        uint32_t cur, uint32_t sort_period, uint32_t mr_j,
-                                                       unsigned long long* digests, uint32_t profile) {
+                                                       unsigned long long* digests, uint32_t profile,
+                                                       uint32_t variant, uint32_t big_above, uint32_t chunk_parity) {
     __shared__ uint32_t red[33];
     __shared__ uint32_t sh_n_slots[2];
     __shared__ unsigned long long sh_prof[8];
     const Who me = who();
+    // Adaptive CTA size (variant 0 / 1; 2 = unconditional): both instantiations are enqueued for
+    // every chunk of steps and the one the previous chunk did not ask for returns at once.  The
+    // word read was written by the previous chunk; this chunk's verdict goes to the other word.
+    if (variant != 2u) {
+        if (me.t == 0) red[0] = __ldcg(&c.dyn->prefer_big[chunk_parity]);
+        __syncthreads();
+        if (red[0] != variant) return;
+        __syncthreads();
+    }
     unsigned int target = 0;
     uint32_t n_upd = 0;
     PhaseClock clk;
@@ -315,6 +330,9 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
         atomicMax(&c.dyn->prof[7], sh_prof[0]);
         if (me.cta == 0) c.dyn->prof[6] += n;
     }
+    // more warps pay once a CTA has more than one round of tiles at the small size
+    if (variant != 2u && me.cta == 0 && me.t == 0)
+        c.dyn->prefer_big[chunk_parity ^ 1u] = sh_n_slots[n & 1] > big_above ? 1u : 0u;
     n_upd = block_sum(n_upd, red);
     if (me.t == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
 }
@@ -562,7 +580,7 @@ extern "C" int ts_reset(ts_sim* s) {
     CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, st));
     k_init<<<std::max(1u, std::min(1184u, (L.V + 255) / 256)), 256, 0, st>>>(s->ctx);
     CUDA_TRY(cudaGetLastError());
-    s->k = 0; s->cur = 0; s->sticky = 0;
+    s->k = 0; s->cur = 0; s->sticky = 0; s->chunk_no = 0;
     return TS_OK;
 }
 
@@ -682,6 +700,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     cudaGetDevice(&dev_id);
     cudaDeviceGetAttribute(&s->sms, cudaDevAttrMultiProcessorCount, dev_id);
     cudaDeviceGetAttribute(&s->smem_limit, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_id);
+    cudaDeviceGetAttribute(&s->l2_bytes, cudaDevAttrL2CacheSize, dev_id);
     bool attr_ok = true;
     for (int t : {512, 640, 768, 896, 1024})
         attr_ok = attr_ok && cudaFuncSetAttribute(step_kernel(t, s->L.emissions != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) == cudaSuccess;
@@ -708,9 +727,20 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
     } else if (!strcmp(key, "blocks_per_sm")) {
         if (value < 1 || value * s->threads > 2048) return fail(TS_EINVAL, "blocks_per_sm * threads must be in 1..2048");
         s->blocks_per_sm = (int)value;
+        s->adaptive = 0;
+    } else if (!strcmp(key, "adaptive_chunk")) {
+        if (value < 1 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "adaptive_chunk must be >= 1");
+        s->adaptive_chunk = (uint32_t)value;
+    } else if (!strcmp(key, "adaptive_above")) {
+        if (value < -1 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "adaptive_above must be >= -1");
+        s->adaptive_above = value;
+    } else if (!strcmp(key, "adaptive")) {
+        s->adaptive = value ? 1 : 0;
+        if (s->adaptive) { s->threads = 640; s->blocks_per_sm = 1; }
     } else if (!strcmp(key, "threads")) {
         if (value < 64 || value > 1024 || value % 32) return fail(TS_EINVAL, "threads must be a multiple of 32 in 64..1024");
         s->threads = (int)value;
+        s->adaptive = 0;
         s->blocks_per_sm = std::min(s->blocks_per_sm, 2048 / s->threads);
     } else if (!strcmp(key, "profile")) {
         s->profile = value ? 1u : 0u;
@@ -729,23 +759,56 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
     const uint32_t R = s->sort_period;
     const uint32_t sorts = R ? (s->k + n) / R - s->k / R : 0;       // steps k with (k + 1) % R == 0
     if (s->mode == 1) {
-        // shared memory holds the move records of the first mr_j slots of every thread
-        const int per_sm_smem = (s->smem_limit - 1024) / s->blocks_per_sm - 1024;
-        uint32_t mr_j = (uint32_t)std::max(0, per_sm_smem / (16 * s->threads));
-        const uint32_t grid = (uint32_t)(s->sms * s->blocks_per_sm);
-        const uint32_t need_j = (s->L.cap + grid * s->threads - 1) / (grid * s->threads);
-        mr_j = std::min(mr_j, need_j);
-        const size_t smem = (size_t)mr_j * 16 * s->threads;
-        const int per_sm_threads = s->threads * s->blocks_per_sm;
-        const void* kern = step_kernel(per_sm_threads, s->L.emissions != 0);
-        int per_sm = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, s->threads, smem));
-        if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, s->threads);
-        CUDA_TRY(cudaMemsetAsync(s->ctx.barrier, 0, 4, st));
-        uint32_t k0 = s->k, cur = s->cur;
-        void* args[] = {&s->ctx, &k0, &n, &cur, (void*)&R, &mr_j, &d_digests, &s->profile};
-        CUDA_TRY(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(s->threads), args, smem, st));
-        if (sorts & 1) s->cur ^= 1;
+        // one cooperative launch of `m` steps from step k0 with CTAs of `threads` threads
+        auto launch = [&](uint32_t k0, uint32_t m, uint32_t cur, int threads, uint32_t variant,
+                          unsigned long long* dig, uint32_t parity) -> int {
+            // shared memory holds the move records of the first mr_j slots of every thread
+            const int per_sm_smem = (s->smem_limit - 1024) / s->blocks_per_sm - 1024;
+            uint32_t mr_j = (uint32_t)std::max(0, per_sm_smem / (16 * threads));
+            const uint32_t grid = (uint32_t)(s->sms * s->blocks_per_sm);
+            const uint32_t need_j = (s->L.cap + grid * threads - 1) / (grid * threads);
+            mr_j = std::min(mr_j, need_j);
+            const size_t smem = (size_t)mr_j * 16 * threads;
+            const void* kern = step_kernel(threads * s->blocks_per_sm, s->L.emissions != 0);
+            int per_sm = 0;
+            CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
+            if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, threads);
+            CUDA_TRY(cudaMemsetAsync(s->ctx.barrier, 0, 4, st));
+            // More warps pay once a CTA has more than one round of tiles at the small size -- as long
+            // as the atlas is L2-resident.  Where its gathers miss L2 (config 4: 460 MB) more warps
+            // measured slower (8.95 against 10.06 G vehicle-updates/s), so the small size stays.
+            const bool atlas_in_l2 = s->L.atlas_chunks * 144ull <= (unsigned long long)s->l2_bytes;
+            uint32_t big_above = s->adaptive_above >= 0 ? (uint32_t)s->adaptive_above
+                                 : atlas_in_l2 ? (uint32_t)s->sms * 640u : 0xFFFFFFFFu;
+            void* args[] = {&s->ctx, &k0, &m, &cur, (void*)&R, &mr_j, &dig, &s->profile, &variant, &big_above, &parity};
+            CUDA_TRY(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, st));
+            return TS_OK;
+        };
+        if (!s->adaptive || s->profile) {           // the phase clocks are per launch: keep it one
+            int rc = launch(s->k, n, s->cur, s->threads, 2u, d_digests, 0u);
+            if (rc) return rc;
+            if (sorts & 1) s->cur ^= 1;
+        } else {
+            // Adaptive CTA size without a host round trip: the steps go out in chunks, each chunk as
+            // TWO launches (640 threads, spill-free, best while a step is one warp's latency; 896
+            // threads, more warps, best once CTAs hold several rounds of tiles); the device runs the
+            // one the previous chunk asked for (Dyn::prefer_big) and the other returns at once.
+            // Results do not depend on the launch geometry.
+            const uint32_t chunk = s->adaptive_chunk;
+            uint32_t k = s->k, cur = s->cur;
+            for (uint32_t done = 0; done < n;) {
+                const uint32_t m = std::min(n - done, chunk);
+                unsigned long long* dig = d_digests ? d_digests + done : nullptr;
+                const uint32_t parity = s->chunk_no++ & 1u;
+                int rc = launch(k, m, cur, 640, 0u, dig, parity);
+                if (rc) return rc;
+                if ((rc = launch(k, m, cur, 896, 1u, dig, parity))) return rc;
+                const uint32_t srt = R ? (k + m) / R - k / R : 0;
+                if (srt & 1) cur ^= 1;
+                k += m; done += m;
+            }
+            s->cur = cur;
+        }
     } else {
         const int g = s->sms * 8, gs = std::min<int>(s->sms * 8, (int)kMaxCtas);
         for (uint32_t i = 0; i < n; i++) {

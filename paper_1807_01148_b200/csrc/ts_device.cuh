@@ -69,6 +69,11 @@ struct Dyn {
     // option "profile": nanoseconds CTA 0 spent in { phase 1, barrier 1, phase 2, barrier 2,
     // compaction + re-sort, digest }, and the number of steps they cover
     unsigned long long prof[8];
+    // adaptive CTA size: which of the two instantiations enqueued for a chunk of steps should run
+    // (0 = the spill-free small one, 1 = the one with more warps).  Chunk c reads word c & 1 and
+    // writes the other one, so the second launch of a chunk never sees the first one's verdict on
+    // the NEXT chunk; see run_steps()
+    uint32_t prefer_big[2];
 };
 
 struct Params {

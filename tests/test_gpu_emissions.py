@@ -24,6 +24,7 @@ def test_config1_full(cfg1, mode):
 @pytest.mark.parametrize("options", [
     dict(sort_period=0), dict(sort_period=1), dict(sort_period=7, threads=128),
     dict(sort_period=50, threads=512, blocks_per_sm=2), dict(sort_period=3, threads=64),
+    dict(adaptive_chunk=50, adaptive_above=700),
 ])
 def test_totals_do_not_depend_on_slot_order(options):
     """The pair is indexed by vehicle id, so compaction, the re-sort and the launch geometry

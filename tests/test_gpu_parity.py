@@ -65,13 +65,16 @@ def test_mixed_controls(mode):
     dict(sort_period=7, threads=128),          # several slots per thread, ragged tile tails
     dict(sort_period=50, threads=512, blocks_per_sm=2),
     dict(sort_period=3, threads=64),           # move records overflow shared memory into global
+    dict(adaptive_chunk=37, adaptive_above=0),     # adaptive CTA size: 896 threads from the second chunk on
+    dict(adaptive_chunk=50, adaptive_above=700),   # ... switching both ways as the slot count crosses 700
+    dict(adaptive_chunk=1, adaptive_above=300, sort_period=5),
 ])
 def test_results_do_not_depend_on_slot_order(options):
     """A9/A10: compaction and the edge re-sort change where a vehicle's state lives, never what
     it is; neither does the launch geometry."""
     b = small_signal_grid()
     _compare(b, b["steps"], 1, **options)
-    if options["sort_period"] in (0, 1):
+    if options.get("sort_period") in (0, 1):
         _compare(b, 400, 0, sort_period=options["sort_period"])
 
 
