@@ -59,6 +59,8 @@ def lib():
         L.orc_fuel_rate.argtypes = [C.c_float, C.c_float]
         L.orc_get_counters.restype = None
         L.orc_get_counters.argtypes = [C.c_void_p, C.POINTER(OrcCounters)]
+        L.orc_set_threads.restype = None
+        L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
         L.orc_destroy.restype = None
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_last_error.restype = C.c_char_p
@@ -108,6 +110,10 @@ class Oracle:
                                *[_ptr(a) for a in k[9:]], C.byref(self._p))
         if not self._h:
             raise OracleError(L.orc_last_error().decode())
+
+    def set_threads(self, n):
+        """Host threads for the intent loop (results do not depend on it; default 1)."""
+        lib().orc_set_threads(self._h, int(n))
 
     def step(self, n, digests=False, check=0, order_seed=0):
         d = np.zeros(n, np.uint64) if digests else None

@@ -2,7 +2,7 @@
 
     python -m oracle.build
 
-gcc, C99, -O2, no FMA contraction, no fast-math: fp32 results are those of the written
+gcc, C99, -O2, no FMA contraction, no fast-math (-fopenmp only serves orc_set_threads): fp32 results are those of the written
 sequence of single operations (reading R21)."""
 import os
 import subprocess
@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "ts_oracle.c")
 LIB = os.path.join(HERE, "libts_oracle.so")
 FLAGS = ["-std=c99", "-O2", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-Wextra",
-         "-fPIC", "-shared"]
+         "-fPIC", "-shared", "-fopenmp"]
 
 
 def build(force=False):

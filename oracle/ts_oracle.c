@@ -15,6 +15,9 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 enum { ST_PENDING = 0, ST_ACTIVE = 1, ST_ARRIVED = 2 };
 enum { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2 };
@@ -78,6 +81,7 @@ struct orc_sim {
     uint32_t n_pending, n_active, n_arrived;
     uint64_t sum_arrive_step;
     orc_counters cnt;
+    int threads;                   /* host threads for the intent loop of step 2 (orc_set_threads) */
 };
 
 /* ---------------------------------------------------------------- scalar building blocks */
@@ -331,6 +335,7 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
     S->exit_steps_sum = xcalloc(E, 8); S->sample_speedcode_sum = xcalloc(E, 8);
     S->co_g = xcalloc(V, 4); S->fuel_ml = xcalloc(V, 4);
     S->n_pending = V;
+    S->threads = 1;
     return S;
 }
 
@@ -376,7 +381,7 @@ static void lane_neighbours(const orc_sim *S, uint64_t g, int32_t c_from, int32_
 }
 
 /* intent of ACTIVE vehicle i from state k only. */
-static void vehicle_intent(orc_sim *S, uint32_t i) {
+static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
     const orc_params *p = &S->p;
     const uint64_t k = S->k;
     const uint32_t e = S->edge[i];
@@ -403,7 +408,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
                     orc_signal_green(S->sig_green[h], S->sig_allred[h], S->sig_offset[h],
                                      S->node_n_in[h], S->edge_in_rank[e], k);
     const int32_t c = cell_of(S, i);
-    S->cnt.updates++;
+    cnt->updates++;
 
     /* 2b own leader: nearest occupied cell with c < cL <= min(C-1, c+H) */
     int has_lead = 0, lead_on_edge = 0;
@@ -417,9 +422,9 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
             s_lead = (float)cL - len;           /* E3 same edge */
             s_lead = s_lead - x;
             dv_lead = v - orc_speed_decode(orc_speed_code(S->v[j]));
-            S->cnt.own_cells += (uint64_t)(cL - c);
+            cnt->own_cells += (uint64_t)(cL - c);
         } else {
-            S->cnt.own_cells += (uint64_t)(lim - c);
+            cnt->own_cells += (uint64_t)(lim - c);
             int32_t Hp = H - (C - 1 - c);
             if (!last && may_cross && Hp > 0) {
                 int32_t C2 = (int32_t)S->edge_len[e2];
@@ -432,9 +437,9 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
                     s_lead = s_lead + (float)cL2;
                     s_lead = s_lead - len;
                     dv_lead = v - orc_speed_decode(orc_speed_code(S->v[j2]));
-                    S->cnt.next_cells += (uint64_t)(cL2 + 1);
+                    cnt->next_cells += (uint64_t)(cL2 + 1);
                 } else {
-                    S->cnt.next_cells += (uint64_t)(lim2 + 1);
+                    cnt->next_cells += (uint64_t)(lim2 + 1);
                 }
             }
         }
@@ -454,7 +459,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
         if (lti >= 0 && lti < (int32_t)lanes_e && x >= (float)p->entry_zone_cells && n < Cf &&
             ((k >> 1) + i) % p->lc_period == 0) {
             lt = (uint32_t)lti;
-            S->cnt.lc_evals++;
+            cnt->lc_evals++;
             int32_t jl, jf;
             lane_neighbours(S, S->lane_base[e] + lt, c, &jl, &jf);
             int32_t lim = c + H < C - 1 ? c + H : C - 1;
@@ -467,15 +472,15 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
                 vLt = orc_speed_decode(orc_speed_code(S->v[jl]));
                 s_Lt = (float)cLt - len;
                 s_Lt = s_Lt - x;
-                S->cnt.lc_cells += (uint64_t)(cLt - c + 1);
-            } else S->cnt.lc_cells += (uint64_t)(lim - c + 1);
+                cnt->lc_cells += (uint64_t)(cLt - c + 1);
+            } else cnt->lc_cells += (uint64_t)(lim - c + 1);
             if (jf != NONE && cell_of(S, (uint32_t)jf) >= lo) {
                 has_F = 1; cF = cell_of(S, (uint32_t)jf);
                 vF = orc_speed_decode(orc_speed_code(S->v[jf]));
                 s_lag = x - len;                /* E3 lag */
                 s_lag = s_lag - (float)(cF + 1);
-                S->cnt.lc_cells += (uint64_t)(c - cF);
-            } else S->cnt.lc_cells += (uint64_t)(c - lo);
+                cnt->lc_cells += (uint64_t)(c - cF);
+            } else cnt->lc_cells += (uint64_t)(c - lo);
 
             int ok = 1;
             float aF_new = 0.0f;
@@ -495,7 +500,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
                 float rem = Cf - x;
                 int mandatory = !last && l >= lanes_e2 && lt < l && rem <= S->mand_dist[i];
                 at_c = idm(S, v, v0, has_Lt, s_Lt, v - vLt);
-                if (mandatory) { accepted = 1; S->cnt.lc_mandatory++; }
+                if (mandatory) { accepted = 1; cnt->lc_mandatory++; }
                 else if (!last && lt >= lanes_e2 && rem <= S->mand_dist[i]) accepted = 0;
                 else {
                     float a_c = lead_on_edge ? idm(S, v, v0, 1, s_lead, dv_lead)
@@ -512,7 +517,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
                     accepted = inc > p->lc_threshold;
                 }
             }
-            if (accepted) S->cnt.lc_accepts++;
+            if (accepted) cnt->lc_accepts++;
         }
     }
 
@@ -532,7 +537,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
     float dx = v + vt;
     dx = 0.5f * dx;
     dx = dx * p->dt;
-    if (dx > cap) { dx = cap; vt = 0.0f; S->cnt.cap_bound++; }
+    if (dx > cap) { dx = cap; vt = 0.0f; cnt->cap_bound++; }
     float xt = x + dx;
 
     /* section 6.3.4: "since it has the position, speed, acceleration of each
@@ -558,14 +563,23 @@ static void vehicle_intent(orc_sim *S, uint32_t i) {
     if (xt >= Cf) {
         if (last) act = ACT_ARRIVE;
         else if (may_cross) {
-            act = ACT_CROSS;
-            claim_lane(S, S->lane_base[e2] + l2, i);
-            if (S->node_ctrl[h] == CTRL_PRIORITY) claim_node(S, h, i);
-        } else { xt = Cf - 0.0625f; vt = 0.0f; S->cnt.held_red++; }
+            act = ACT_CROSS;                    /* its claims are posted by post_claims() */
+        } else { xt = Cf - 0.0625f; vt = 0.0f; cnt->held_red++; }
     }
     S->xt[i] = xt; S->vt[i] = vt; S->act[i] = act;
     S->ln[i] = (uint8_t)(accepted ? lt : l);
     S->e2[i] = e2; S->l2[i] = (uint8_t)l2;
+}
+
+/* SURVEY.md 8(c) step 2f, second half: a CROSS intent claims its target lane and, at a PRIORITY
+ * node, the node (claim = minimum id).  Kept apart from vehicle_intent() so that the intents,
+ * which read state k only and write only the vehicle's own intent (I8), may be evaluated by
+ * several host threads (orc_set_threads); the claims are posted by one thread. */
+static void post_claims(orc_sim *S, uint32_t i) {
+    if (S->act[i] != ACT_CROSS) return;
+    uint32_t h = S->edge_to[S->edge[i]];
+    claim_lane(S, S->lane_base[S->e2[i]] + S->l2[i], i);
+    if (S->node_ctrl[h] == CTRL_PRIORITY) claim_node(S, h, i);
 }
 
 /* departure intent of queue q. */
@@ -718,6 +732,37 @@ static void shuffle_active(orc_sim *S, uint64_t seed) {
     }
 }
 
+/* The intent loop of step 2 on S->threads host threads (OpenMP).  Licensed by the synchronous
+ * update: vehicle_intent() reads state k and writes only vehicle i's own intent, so the loop's
+ * iterations are independent (the same property as I8).  The arithmetic is vehicle_intent()'s,
+ * untouched; work counters are kept per thread and added up.  Used only to get through the
+ * multi-hour whole-run traces of tests/golden/make_golden.py; the default is one thread. */
+static void intents_threaded(orc_sim *S) {
+    enum { MAXT = 64 };
+    static orc_counters zero;
+    orc_counters part[MAXT];
+    int T = S->threads > MAXT ? MAXT : S->threads;
+    for (int t = 0; t < T; t++) part[t] = zero;
+    long n_act = (long)S->n_active_list;
+#ifdef _OPENMP
+#pragma omp parallel num_threads(T)
+    {
+        orc_counters *cnt = &part[omp_get_thread_num()];
+#pragma omp for schedule(static)
+        for (long n = 0; n < n_act; n++) vehicle_intent(S, S->active[n], cnt);
+    }
+#else
+    for (long n = 0; n < n_act; n++) vehicle_intent(S, S->active[n], &part[0]);
+#endif
+    uint64_t *dst = (uint64_t *)&S->cnt;
+    for (int t = 0; t < T; t++) {
+        const uint64_t *src = (const uint64_t *)&part[t];
+        for (size_t f = 0; f < sizeof(orc_counters) / 8; f++) dst[f] += src[f];
+    }
+}
+
+void orc_set_threads(orc_sim *S, int n) { S->threads = n < 1 ? 1 : n; }
+
 static int one_step(orc_sim *S, int check, uint64_t order_seed) {
     const uint64_t k = S->k;
     const uint32_t k1 = (uint32_t)(k + 1);
@@ -726,7 +771,9 @@ static int one_step(orc_sim *S, int check, uint64_t order_seed) {
 
     /* steps 1-3: intents from state k */
     S->n_touched_lanes = 0; S->n_touched_nodes = 0;
-    for (uint32_t n = 0; n < S->n_active_list; n++) vehicle_intent(S, S->active[n]);
+    if (S->threads > 1) intents_threaded(S);
+    else for (uint32_t n = 0; n < S->n_active_list; n++) vehicle_intent(S, S->active[n], &S->cnt);
+    for (uint32_t n = 0; n < S->n_active_list; n++) post_claims(S, S->active[n]);
     for (uint32_t q = 0; q < S->n_queues; q++) departure_intent(S, q);
 
     /* step 4: resolve + commit.  Only own intent and the claim words are read here. */

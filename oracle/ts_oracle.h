@@ -127,6 +127,13 @@ float orc_co_rate(float v);
 float orc_fuel_rate(float v, float acc);
 
 void orc_get_counters(const orc_sim *s, orc_counters *out);
+
+/* Host threads for the intent loop of step 2 (default 1 = the plain sequential program).
+ * Every intent reads state k only and writes only its own vehicle's intent, so the loop's
+ * iterations are independent; results are identical for every n (tests/test_oracle_invariants.py).
+ * Exists so that tests/golden/make_golden.py can get through the whole run of config 4
+ * (5.4e10 vehicle-updates); bench.py's cpu_baseline times the default. */
+void orc_set_threads(orc_sim *s, int n);
 void orc_destroy(orc_sim *s);
 const char *orc_last_error(void);
 

@@ -69,6 +69,27 @@ def test_i8_order_independence(cfg1):
     assert (Oracle(b2).step(600, digests=True) == Oracle(b2).step(600, digests=True, order_seed=99)).all()
 
 
+def test_threaded_intent_loop_changes_nothing():
+    """orc_set_threads(n): the intent loop of step 2 on n host threads (used by make_golden.py for
+    the multi-hour traces) gives the same digests, state, edge statistics, emission totals and
+    work counters as the sequential program, with the invariant checks on."""
+    b = small_signal_grid(n_vehicles=1200, steps=900)
+    b = dict(b, params=dict(b["params"], emissions=1))
+    one, many = Oracle(b), Oracle(b)
+    many.set_threads(5)
+    assert (one.step(900, digests=True, check=1) == many.step(900, digests=True, check=1)).all()
+    assert one.counters() == many.counters()
+    s1, s2 = one.read_state(), many.read_state()
+    for k in s1:
+        assert np.array_equal(s1[k], s2[k]), k
+    e1, e2 = one.read_edge_stats(), many.read_edge_stats()
+    for k in e1:
+        assert np.array_equal(e1[k], e2[k]), k
+    m1, m2 = one.read_emissions(), many.read_emissions()
+    assert np.array_equal(m1["co_g"].view(np.uint32), m2["co_g"].view(np.uint32))
+    assert np.array_equal(m1["fuel_ml"].view(np.uint32), m2["fuel_ml"].view(np.uint32))
+
+
 def test_digest_sensitivity(cfg1):
     """The digest separates runs that differ in one parameter (it is not constant)."""
     b = dict(cfg1); b["params"] = dict(cfg1["params"], T=1.6)
