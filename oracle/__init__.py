@@ -20,7 +20,13 @@ _PARAM_FIELDS = [
     ("lookahead_cells", C.c_uint32), ("lookback_cells", C.c_uint32), ("lc_period", C.c_uint32),
     ("entry_zone_cells", C.c_uint32), ("insert_clear_cells", C.c_uint32),
     ("sample_period_steps", C.c_uint32), ("emissions", C.c_uint32),
+    ("n_types", C.c_uint32), ("type_len", C.c_float * 4), ("type_a", C.c_float * 4),
+    ("type_vmax", C.c_float * 4), ("amber_steps", C.c_uint32), ("stop_dist", C.c_float),
+    ("stop_speed", C.c_float),
 ]
+# fields that may be absent from a params dict, with the value that switches the feature off
+_OPTIONAL = dict(emissions=0, n_types=0, type_len=(), type_a=(), type_vmax=(), amber_steps=0,
+                 stop_dist=4.0, stop_speed=0.5)
 
 
 class OrcParams(C.Structure):
@@ -44,7 +50,7 @@ def lib():
     if _lib is None:
         L = C.CDLL(_build())
         L.orc_create.restype = C.c_void_p
-        L.orc_create.argtypes = [C.c_uint32, C.c_uint32] + [C.c_void_p] * 9 + [C.c_uint32] + [C.c_void_p] * 5 + [C.POINTER(OrcParams)]
+        L.orc_create.argtypes = [C.c_uint32, C.c_uint32] + [C.c_void_p] * 9 + [C.c_uint32] + [C.c_void_p] * 6 + [C.POINTER(OrcParams)]
         L.orc_step.restype = C.c_int
         L.orc_step.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_int, C.c_uint64]
         L.orc_read_state.restype = None
@@ -72,6 +78,8 @@ def lib():
         L.orc_speed_decode.argtypes = [C.c_uint8]
         L.orc_signal_green.restype = C.c_int
         L.orc_signal_green.argtypes = [C.c_uint32] * 5 + [C.c_uint64]
+        L.orc_signal_phase.restype = C.c_int
+        L.orc_signal_phase.argtypes = [C.c_uint32] * 8 + [C.c_uint64]
         L.orc_mix64.restype = C.c_uint64
         L.orc_mix64.argtypes = [C.c_uint64]
         _lib = L
@@ -80,8 +88,11 @@ def lib():
 
 def make_params(d) -> OrcParams:
     p = OrcParams()
-    for name, _ in _PARAM_FIELDS:
-        setattr(p, name, d.get(name, 0) if name == "emissions" else d[name])
+    for name, ctype in _PARAM_FIELDS:
+        val = d.get(name, _OPTIONAL[name]) if name in _OPTIONAL else d[name]
+        if name.startswith("type_"):
+            val = ctype(*[float(x) for x in val])
+        setattr(p, name, val)
     return p
 
 
@@ -105,6 +116,7 @@ class Oracle:
             "edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim", "node_ctrl",
             "sig_green_steps", "sig_allred_steps", "sig_offset_steps", "route_off", "route_edges",
             "depart_time_s", "v0_mult", "mand_dist_m")]
+        self._keep.append(None if b.get("veh_type") is None else np.ascontiguousarray(b["veh_type"], np.uint8))
         k = self._keep
         self._h = L.orc_create(int(b["n_nodes"]), self.E, *[_ptr(a) for a in k[:9]], self.V,
                                *[_ptr(a) for a in k[9:]], C.byref(self._p))

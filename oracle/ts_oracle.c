@@ -20,7 +20,9 @@
 #endif
 
 enum { ST_PENDING = 0, ST_ACTIVE = 1, ST_ARRIVED = 2 };
-enum { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2 };
+enum { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2, CTRL_STOP = 3, CTRL_SIGNAL_NM = 4 };
+enum { SIG_RED = 0, SIG_GREEN = 1, SIG_AMBER = 2 };
+#define MAX_TYPES 4
 enum { ACT_STAY = 0, ACT_ARRIVE = 1, ACT_CROSS = 2 };
 #define NONE (-1)
 #define NO_CLAIM 0xFFFFFFFFu
@@ -31,14 +33,25 @@ const char *orc_last_error(void) { return g_err; }
 
 struct orc_sim {
     orc_params p;
-    float Kinv;                    /* 1 / (2*sqrtf(a*b)), fp32, computed once (reading R27) */
+    /* per vehicle type ("a second type of vehicle to represent trucks ... size,
+     * acceleration, and maximum speed"; reading R31): length, acceleration ability a, 1/(2 sqrt(a b))
+     * (fp32, computed once, reading R27), speed cap */
+    uint32_t n_types;
+    float t_len[MAX_TYPES], t_a[MAX_TYPES], t_Kinv[MAX_TYPES], t_vmax[MAX_TYPES];
+    float two_b;                   /* 2*b, fp32, computed once (amber rule, reading R36) */
+    uint8_t *veh_type;             /* [V] */
     uint32_t N, E, V;
     /* network */
     uint32_t *edge_from, *edge_to, *edge_len;
-    uint8_t *edge_lanes, *edge_in_rank;
+    uint8_t *edge_lanes, *edge_in_rank, *edge_out_rank;
     float *edge_vlim;
     uint8_t *node_ctrl;
-    uint32_t *node_n_in, *sig_green, *sig_allred, *sig_offset;
+    uint32_t *node_n_in, *node_n_out, *sig_green, *sig_allred, *sig_offset;
+    /* CTRL_STOP (reading R34): first step at which the node is free again; UINT32_MAX while a
+     * vehicle that crossed it has not yet cleared it with its rear bumper */
+    uint32_t *node_free_from;
+    uint8_t *made_stop, *owns_node; /* [V] has come to a halt at the stop line of its edge / holds the node at its edge's tail */
+    uint8_t *stop_t;               /* [V] intent: made_stop after this step */
     uint64_t *lane_base;           /* [E+1] global lane index of (e,0) */
     /* demand */
     uint64_t *route_off;
@@ -103,17 +116,18 @@ float orc_speed_decode(uint8_t code) { return (float)((int)code - 1) * 0.25f; }
  * Reading R27: the two quotients whose divisor does not depend on the traffic are
  * formed with a reciprocal rounded once -- v/v0 as v * (1/v0), v dv/(2 sqrt(ab)) as (v dv) * (1/K)
  * -- each still one rounding per written operation; s* / s stays a division. */
-static float idm(const orc_sim *S, float v, float v0, int has, float s, float dv) {
+static float idm(const orc_sim *S, uint32_t ty, float v, float v0, int has, float s, float dv) {
     const orc_params *p = &S->p;
+    const float a = S->t_a[ty];        /* "a is the acceleration ability of the vehicle" */
     float rinv = 1.0f / v0;
     float r = v * rinv;
     float r2 = r * r;
     float r4 = r2 * r2;
     float fr = 1.0f - r4;
-    if (!has) return p->a * fr;
+    if (!has) return a * fr;
     float t = v * p->T;
     float u = v * dv;
-    float w = u * S->Kinv;
+    float w = u * S->t_Kinv[ty];
     t = t + w;
     t = fmaxf(t, 0.0f);
     float ss = p->s0 + t;
@@ -121,15 +135,15 @@ static float idm(const orc_sim *S, float v, float v0, int has, float s, float dv
     float q = ss / se;
     float q2 = q * q;
     float d = fr - q2;
-    return p->a * d;
+    return a * d;
 }
 
 float orc_idm(const orc_params *p, float v, float v0, int has_leader, float s, float dv) {
     orc_sim tmp;
     tmp.p = *p;
     float ab = p->a * p->b;
-    { float K = 2.0f * sqrtf(ab); tmp.Kinv = 1.0f / K; }
-    return idm(&tmp, v, v0, has_leader, s, dv);
+    { float K = 2.0f * sqrtf(ab); tmp.t_Kinv[0] = 1.0f / K; tmp.t_a[0] = p->a; }
+    return idm(&tmp, 0, v, v0, has_leader, s, dv);
 }
 
 /* CO emission rate, Eq. 8 (Stein and Walker 2003):
@@ -186,6 +200,24 @@ int orc_signal_green(uint32_t green, uint32_t allred, uint32_t offset, uint32_t 
     return (t / P == in_rank) && (t % P < green);
 }
 
+/* The same plan with an amber interval after the green (reading R36) and, for n_out > 0, the
+ * paper's literal phasing ("given an intersection with n inbound edges and m outbound,
+ * our system creates the geometric combination nm of necessary traffic phasing ... in a round robing
+ * logic"; reading R35): one phase per MOVEMENT (inbound edge i, outbound edge j), in the order
+ * i*m + j, each green + amber + allred steps long.  n_out == 0: one phase per inbound edge (R16). */
+int orc_signal_phase(uint32_t green, uint32_t amber, uint32_t allred, uint32_t offset, uint32_t n_in,
+                     uint32_t n_out, uint32_t in_rank, uint32_t out_rank, uint64_t k) {
+    uint64_t P = (uint64_t)green + amber + allred;
+    uint64_t n_phases = n_out ? (uint64_t)n_in * n_out : n_in;
+    uint64_t mine = n_out ? (uint64_t)in_rank * n_out + out_rank : in_rank;
+    uint64_t t = (k + offset) % (n_phases * P);
+    if (t / P != mine) return SIG_RED;
+    uint64_t pos = t % P;
+    if (pos < green) return SIG_GREEN;
+    if (pos < (uint64_t)green + amber) return SIG_AMBER;
+    return SIG_RED;
+}
+
 /* SplitMix64 finaliser. */
 uint64_t orc_mix64(uint64_t z) {
     z += 0x9E3779B97F4A7C15ull;
@@ -226,14 +258,25 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
                     const uint32_t *sig_offset_steps,
                     uint32_t n_vehicles, const uint64_t *route_off,
                     const uint32_t *route_edges, const float *depart_time_s,
-                    const float *v0_mult, const float *mand_dist_m,
+                    const float *v0_mult, const float *mand_dist_m, const uint8_t *veh_type,
                     const orc_params *params) {
     const orc_params *p = params;
     g_err[0] = 0;
     if (!(p->dt > 0) || !(p->a > 0) || !(p->b > 0) || !(p->T >= 0) || !(p->s0 >= 0) ||
         !(p->veh_len >= 2.0f) || p->lookahead_cells == 0 || p->lookahead_cells % 16 ||
-        p->insert_clear_cells == 0 || p->insert_clear_cells > 16) {
+        p->insert_clear_cells == 0 || p->insert_clear_cells > 16 || p->n_types > MAX_TYPES) {
         FAIL("bad params"); return NULL;
+    }
+    /* vehicle types (reading R31): none given = one type {veh_len, a, no speed cap} */
+    uint32_t n_types = p->n_types ? p->n_types : 1;
+    float max_len = 0.0f, max_a = 0.0f;
+    for (uint32_t t = 0; t < n_types; t++) {
+        float len_t = p->n_types ? p->type_len[t] : p->veh_len;
+        float a_t = p->n_types ? p->type_a[t] : p->a;
+        float vmax_t = p->n_types ? p->type_vmax[t] : INFINITY;
+        if (!(len_t >= 2.0f) || !(a_t > 0) || !(vmax_t > 0)) { FAIL("vehicle type %u", t); return NULL; }
+        if (len_t > max_len) max_len = len_t;
+        if (a_t > max_a) max_a = a_t;
     }
     float max_mult = 1.0f;
     for (uint32_t i = 0; i < n_vehicles; i++) {
@@ -243,20 +286,33 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
         }
         if (!(depart_time_s[i] >= 0)) { FAIL("depart_time_s[%u] < 0", i); return NULL; }
         if (route_off[i + 1] <= route_off[i]) { FAIL("route %u empty", i); return NULL; }
+        if (veh_type && veh_type[i] >= n_types) { FAIL("veh_type[%u]", i); return NULL; }
     }
+    float max_vlim = 0.0f;
     for (uint32_t e = 0; e < n_edges; e++) {
+        if (edge_vlim[e] > max_vlim) max_vlim = edge_vlim[e];
         if (edge_from[e] >= n_nodes || edge_to[e] >= n_nodes) { FAIL("edge %u endpoint", e); return NULL; }
         if (edge_len_m[e] < 16 || edge_len_m[e] > 65535) { FAIL("edge %u length", e); return NULL; }
         if (edge_lanes[e] < 1 || edge_lanes[e] > 8) { FAIL("edge %u lanes", e); return NULL; }
         if (!(edge_vlim[e] > 0)) { FAIL("edge %u vlim", e); return NULL; }
         /* a vehicle entering an edge must land short of the zone where lanes may be changed */
-        double adv = (double)edge_vlim[e] * max_mult * p->dt + 0.5 * p->a * p->dt * p->dt + p->veh_len;
+        double adv = (double)edge_vlim[e] * max_mult * p->dt + 0.5 * max_a * p->dt * p->dt + max_len;
         if (!(adv < (double)p->entry_zone_cells)) { FAIL("edge %u: entry zone too short", e); return NULL; }
     }
-    for (uint32_t h = 0; h < n_nodes; h++) {
-        if (node_ctrl[h] > 2) { FAIL("node %u ctrl", h); return NULL; }
-        if (node_ctrl[h] == CTRL_SIGNAL && sig_green_steps[h] == 0) { FAIL("node %u green", h); return NULL; }
+    {   /* the look-ahead (and the look-back of the lane-change rule) must reach further than a
+         * vehicle can advance in one step plus a vehicle length: nobody jumps over a leader unseen */
+        double adv = (double)max_vlim * max_mult * p->dt + 0.5 * max_a * p->dt * p->dt + max_len;
+        if (!((double)p->lookahead_cells >= adv)) { FAIL("lookahead_cells too short"); return NULL; }
+        if (p->lc_period != 0 && !((double)p->lookback_cells >= adv)) { FAIL("lookback_cells too short"); return NULL; }
     }
+    int any_stop = 0;
+    for (uint32_t h = 0; h < n_nodes; h++) {
+        if (node_ctrl[h] > CTRL_SIGNAL_NM) { FAIL("node %u ctrl", h); return NULL; }
+        if ((node_ctrl[h] == CTRL_SIGNAL || node_ctrl[h] == CTRL_SIGNAL_NM) && sig_green_steps[h] == 0) { FAIL("node %u green", h); return NULL; }
+        if (node_ctrl[h] == CTRL_STOP) any_stop = 1;
+    }
+    /* a vehicle that holds a STOP node lets go once its rear bumper is past it, on the edge it entered */
+    if (any_stop && !(max_len < 16.0f)) { FAIL("STOP control needs vehicle lengths < 16 m"); return NULL; }
     for (uint32_t i = 0; i < n_vehicles; i++)
         for (uint64_t j = route_off[i]; j < route_off[i + 1]; j++) {
             if (route_edges[j] >= n_edges) { FAIL("route %u edge id", i); return NULL; }
@@ -267,7 +323,14 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
 
     orc_sim *S = (orc_sim *)xcalloc(1, sizeof *S);
     S->p = *p;
-    { float ab = p->a * p->b; float K = 2.0f * sqrtf(ab); S->Kinv = 1.0f / K; }
+    S->n_types = n_types;
+    for (uint32_t t = 0; t < n_types; t++) {
+        S->t_len[t] = p->n_types ? p->type_len[t] : p->veh_len;
+        S->t_a[t] = p->n_types ? p->type_a[t] : p->a;
+        S->t_vmax[t] = p->n_types ? p->type_vmax[t] : INFINITY;
+        float ab = S->t_a[t] * p->b; float K = 2.0f * sqrtf(ab); S->t_Kinv[t] = 1.0f / K;
+    }
+    S->two_b = 2.0f * p->b;
     S->N = n_nodes; S->E = n_edges; S->V = n_vehicles;
     uint32_t N = n_nodes, E = n_edges, V = n_vehicles;
     S->edge_from = xdup(edge_from, E, 4); S->edge_to = xdup(edge_to, E, 4);
@@ -277,11 +340,18 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
     S->sig_offset = xdup(sig_offset_steps, N, 4);
     /* in_rank: rank of e among the inbound edges of its head node, by edge index */
     S->node_n_in = xcalloc(N, 4); S->edge_in_rank = xcalloc(E, 1);
+    S->node_n_out = xcalloc(N, 4); S->edge_out_rank = xcalloc(E, 1);
     for (uint32_t e = 0; e < E; e++) {
-        uint32_t h = edge_to[e];
+        uint32_t h = edge_to[e], t = edge_from[e];
         if (S->node_n_in[h] >= 255) { FAIL("node %u in-degree", h); orc_destroy(S); return NULL; }
         S->edge_in_rank[e] = (uint8_t)S->node_n_in[h]++;
+        if (S->node_n_out[t] >= 255) { FAIL("node %u out-degree", t); orc_destroy(S); return NULL; }
+        S->edge_out_rank[e] = (uint8_t)S->node_n_out[t]++;   /* rank among the outbound edges, by edge index */
     }
+    S->node_free_from = xcalloc(N, 4);
+    S->made_stop = xcalloc(V, 1); S->owns_node = xcalloc(V, 1); S->stop_t = xcalloc(V, 1);
+    S->veh_type = xcalloc(V, 1);
+    if (veh_type) memcpy(S->veh_type, veh_type, V);
     S->lane_base = xcalloc((size_t)E + 1, 8);
     for (uint32_t e = 0; e < E; e++) S->lane_base[e + 1] = S->lane_base[e] + edge_lanes[e];
     uint64_t n_lanes = S->lane_base[E];
@@ -355,6 +425,8 @@ void orc_destroy(orc_sim *S) {
     free(S->entry_lane); free(S->cross_node);
     free(S->entered); free(S->exited); free(S->sample_count_sum); free(S->exit_steps_sum);
     free(S->sample_speedcode_sum); free(S->co_g); free(S->fuel_ml);
+    free(S->node_n_out); free(S->edge_out_rank); free(S->node_free_from);
+    free(S->made_stop); free(S->owns_node); free(S->stop_t); free(S->veh_type);
     free(S);
 }
 
@@ -390,11 +462,14 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
     const int32_t C = (int32_t)S->edge_len[e];
     const float Cf = (float)C;
     const int32_t H = (int32_t)p->lookahead_cells, Hb = (int32_t)p->lookback_cells;
-    const float len = p->veh_len;
+    const uint32_t ty = S->veh_type[i];
+    const float len = S->t_len[ty];             /* this vehicle's own length */
+    const float a_i = S->t_a[ty];
     const uint32_t lanes_e = S->edge_lanes[e];
 
-    /* 2a */
-    const float v0 = S->v0_mult[i] * S->edge_vlim[e];
+    /* 2a; a truck's desired speed is capped by its type's maximum (reading R31) */
+    float v0 = S->v0_mult[i] * S->edge_vlim[e];
+    v0 = fminf(v0, S->t_vmax[ty]);
     const uint64_t rpos = S->route_off[i] + S->r[i];
     const int last = (rpos + 1 == S->route_off[i + 1]);
     uint32_t e2 = 0, l2 = 0, lanes_e2 = 0;
@@ -404,9 +479,32 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
         l2 = l < lanes_e2 - 1 ? l : lanes_e2 - 1;
     }
     const uint32_t h = S->edge_to[e];
-    int may_cross = last || S->node_ctrl[h] != CTRL_SIGNAL ||
-                    orc_signal_green(S->sig_green[h], S->sig_allred[h], S->sig_offset[h],
-                                     S->node_n_in[h], S->edge_in_rank[e], k);
+    const uint32_t ctrl = S->node_ctrl[h];
+    int may_cross = 1;
+    uint8_t made_stop = S->made_stop[i];
+    if (!last && (ctrl == CTRL_SIGNAL || ctrl == CTRL_SIGNAL_NM)) {
+        int ph = orc_signal_phase(S->sig_green[h], p->amber_steps, S->sig_allred[h], S->sig_offset[h],
+                                  S->node_n_in[h], ctrl == CTRL_SIGNAL_NM ? S->node_n_out[h] : 0,
+                                  S->edge_in_rank[e], S->edge_out_rank[e2], k);
+        may_cross = ph == SIG_GREEN;
+        if (ph == SIG_AMBER) {
+            /* reading R36: on amber a vehicle goes on iff it could not stop before the line at the
+             * comfortable deceleration b: v^2 > 2 b (C - x) */
+            float rem = Cf - x;
+            float vv = v * v;
+            float need = S->two_b * rem;
+            may_cross = vv > need;
+        }
+    } else if (!last && ctrl == CTRL_STOP) {
+        /* reading R34 ("allows just one vehicle at a time into the intersection and
+         * waits until the car has reached the next edge"): the line is a standing obstacle until
+         * the vehicle has come to a halt at it (within stop_dist of the line at no more than
+         * stop_speed) AND the node is not held by a vehicle that crossed it earlier */
+        float rem = Cf - x;
+        if (rem <= p->stop_dist && v <= p->stop_speed) made_stop = 1;
+        may_cross = made_stop && S->node_free_from[h] <= k;
+    }
+    S->stop_t[i] = made_stop;
     const int32_t c = cell_of(S, i);
     cnt->updates++;
 
@@ -419,7 +517,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
         if (j != NONE && cell_of(S, (uint32_t)j) <= lim) {
             int32_t cL = cell_of(S, (uint32_t)j);
             has_lead = 1; lead_on_edge = 1;
-            s_lead = (float)cL - len;           /* E3 same edge */
+            s_lead = (float)cL - S->t_len[S->veh_type[j]];   /* E3 same edge: the LEADER's length */
             s_lead = s_lead - x;
             dv_lead = v - orc_speed_decode(orc_speed_code(S->v[j]));
             cnt->own_cells += (uint64_t)(cL - c);
@@ -435,7 +533,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
                     has_lead = 1;
                     s_lead = Cf - x;            /* E3 across the node */
                     s_lead = s_lead + (float)cL2;
-                    s_lead = s_lead - len;
+                    s_lead = s_lead - S->t_len[S->veh_type[j2]];
                     dv_lead = v - orc_speed_decode(orc_speed_code(S->v[j2]));
                     cnt->next_cells += (uint64_t)(cL2 + 1);
                 } else {
@@ -452,7 +550,7 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
     if (p->lc_period != 0 && lanes_e >= 2) {
         int dir = (k & 1) ? -1 : +1;
         int32_t lti = (int32_t)l + dir;
-        float n = p->a * p->dt;                 /* E5 cannot cross this step */
+        float n = a_i * p->dt;                  /* E5 cannot cross this step */
         n = v + n;
         n = n * p->dt;
         n = x + n;
@@ -466,16 +564,19 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
             int32_t lo = c - Hb > 0 ? c - Hb : 0;
             int has_F = 0;
             int32_t cLt = 0, cF = 0;
-            float vLt = 0.0f, vF = 0.0f, s_lag = 0.0f;
+            float vLt = 0.0f, vF = 0.0f, s_lag = 0.0f, len_Lt = 0.0f;
+            uint32_t tyF = 0;
             if (jl != NONE && cell_of(S, (uint32_t)jl) <= lim) {
                 has_Lt = 1; cLt = cell_of(S, (uint32_t)jl);
                 vLt = orc_speed_decode(orc_speed_code(S->v[jl]));
-                s_Lt = (float)cLt - len;
+                len_Lt = S->t_len[S->veh_type[jl]];
+                s_Lt = (float)cLt - len_Lt;
                 s_Lt = s_Lt - x;
                 cnt->lc_cells += (uint64_t)(cLt - c + 1);
             } else cnt->lc_cells += (uint64_t)(lim - c + 1);
             if (jf != NONE && cell_of(S, (uint32_t)jf) >= lo) {
                 has_F = 1; cF = cell_of(S, (uint32_t)jf);
+                tyF = S->veh_type[jf];
                 vF = orc_speed_decode(orc_speed_code(S->v[jf]));
                 s_lag = x - len;                /* E3 lag */
                 s_lag = s_lag - (float)(cF + 1);
@@ -484,32 +585,34 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
 
             int ok = 1;
             float aF_new = 0.0f;
+            /* what the changer knows of the lag vehicle's desired speed: the edge limit, capped by its type */
+            float v0F = fminf(S->edge_vlim[e], S->t_vmax[tyF]);
             if (has_Lt && !(s_Lt >= p->s0)) ok = 0;                         /* G1 */
             if (ok && has_F) {                                              /* G2 */
-                float m = 0.5f * p->a;          /* E4 */
+                float m = 0.5f * S->t_a[tyF];   /* E4, with the lag vehicle's acceleration ability */
                 m = m * p->dt;
                 m = (vF + 0.125f) + m;
                 m = m * p->dt;
                 if (!(s_lag >= p->s0 && s_lag >= m)) ok = 0;
             }
             if (ok && has_F) {                                              /* G3 */
-                aF_new = idm(S, vF, S->edge_vlim[e], 1, s_lag, vF - v);
+                aF_new = idm(S, tyF, vF, v0F, 1, s_lag, vF - v);
                 if (!(aF_new >= -p->b_safe)) ok = 0;
             }
             if (ok) {                                                       /* G4 */
                 float rem = Cf - x;
                 int mandatory = !last && l >= lanes_e2 && lt < l && rem <= S->mand_dist[i];
-                at_c = idm(S, v, v0, has_Lt, s_Lt, v - vLt);
+                at_c = idm(S, ty, v, v0, has_Lt, s_Lt, v - vLt);
                 if (mandatory) { accepted = 1; cnt->lc_mandatory++; }
                 else if (!last && lt >= lanes_e2 && rem <= S->mand_dist[i]) accepted = 0;
                 else {
-                    float a_c = lead_on_edge ? idm(S, v, v0, 1, s_lead, dv_lead)
-                                             : idm(S, v, v0, 0, 0.0f, 0.0f);
+                    float a_c = lead_on_edge ? idm(S, ty, v, v0, 1, s_lead, dv_lead)
+                                             : idm(S, ty, v, v0, 0, 0.0f, 0.0f);
                     float inc = at_c - a_c;
                     if (has_F) {
-                        float sF = (float)cLt - len;
+                        float sF = (float)cLt - len_Lt;
                         sF = sF - (float)(cF + 1);
-                        float a_F = idm(S, vF, S->edge_vlim[e], has_Lt, sF, vF - vLt);
+                        float a_F = idm(S, tyF, vF, v0F, has_Lt, sF, vF - vLt);
                         float d2 = aF_new - a_F;
                         d2 = p->politeness * d2;
                         inc = inc + d2;
@@ -522,10 +625,10 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
     }
 
     /* 2e acceleration and integration (E2, reading R3) */
-    float acc = idm(S, v, v0, has_lead, s_lead, dv_lead);
+    float acc = idm(S, ty, v, v0, has_lead, s_lead, dv_lead);
     if (!may_cross) {                            /* 2c stop line as a standing obstacle (R17) */
         float s_stop = Cf - x;
-        acc = fminf(acc, idm(S, v, v0, 1, s_stop, v));
+        acc = fminf(acc, idm(S, ty, v, v0, 1, s_stop, v));
     }
     float cap = INFINITY;
     if (has_lead) cap = fmaxf(s_lead, 0.0f);
@@ -579,7 +682,7 @@ static void post_claims(orc_sim *S, uint32_t i) {
     if (S->act[i] != ACT_CROSS) return;
     uint32_t h = S->edge_to[S->edge[i]];
     claim_lane(S, S->lane_base[S->e2[i]] + S->l2[i], i);
-    if (S->node_ctrl[h] == CTRL_PRIORITY) claim_node(S, h, i);
+    if (S->node_ctrl[h] == CTRL_PRIORITY || S->node_ctrl[h] == CTRL_STOP) claim_node(S, h, i);
 }
 
 /* departure intent of queue q. */
@@ -691,7 +794,7 @@ static int check_invariants(const orc_sim *S) {
     /* I4 speed range, I5 position range, route consistency */
     for (uint32_t n = 0; n < S->n_active_list; n++) {
         uint32_t i = S->active[n], e = S->edge[i];
-        float v0 = S->v0_mult[i] * S->edge_vlim[e];
+        float v0 = fminf(S->v0_mult[i] * S->edge_vlim[e], S->t_vmax[S->veh_type[i]]);
         if (!(S->v[i] >= 0.0f && S->v[i] <= v0)) { FAIL("I4: step %llu veh %u v=%g v0=%g", k, i, S->v[i], v0); return -1; }
         if (!(S->x[i] >= 0.0f && S->x[i] < (float)S->edge_len[e])) { FAIL("I5: step %llu veh %u x=%g C=%u", k, i, S->x[i], S->edge_len[e]); return -1; }
         if (S->route_edges[S->route_off[i] + S->r[i]] != e) { FAIL("I1: step %llu veh %u off route", k, i); return -1; }
@@ -785,19 +888,38 @@ static int one_step(orc_sim *S, int check, uint64_t order_seed) {
         uint64_t g = S->lane_base[e] + l;
         float Cf = (float)S->edge_len[e];
         float x_old = S->x[i], v_old = S->v[i];
+        /* reading R34: a vehicle that holds the STOP node at the tail of its edge lets go once its
+         * rear bumper is past it (always the case by the time it leaves the edge: len < 16 <= C);
+         * the node is free again from the next step on */
+        if (S->owns_node[i] && S->xt[i] >= S->t_len[S->veh_type[i]]) {
+            S->node_free_from[S->edge_from[e]] = k1;
+            S->owns_node[i] = 0;
+        }
+        S->made_stop[i] = S->stop_t[i];
         if (S->act[i] == ACT_CROSS) {
             uint32_t e2 = S->e2[i], l2 = S->l2[i], h = S->edge_to[e];
             uint64_t g2 = S->lane_base[e2] + l2;
+            uint32_t ctrl = S->node_ctrl[h];
             int win = S->lane_claim[g2] == i &&
-                      (S->node_ctrl[h] != CTRL_PRIORITY || S->node_claim[h] == i);
+                      ((ctrl != CTRL_PRIORITY && ctrl != CTRL_STOP) || S->node_claim[h] == i);
             if (win) {
-                if (check && S->node_ctrl[h] == CTRL_SIGNAL &&
-                    !orc_signal_green(S->sig_green[h], S->sig_allred[h], S->sig_offset[h], S->node_n_in[h], S->edge_in_rank[e], k)) {
+                if (check && (ctrl == CTRL_SIGNAL || ctrl == CTRL_SIGNAL_NM) &&
+                    orc_signal_phase(S->sig_green[h], S->p.amber_steps, S->sig_allred[h], S->sig_offset[h], S->node_n_in[h],
+                                     ctrl == CTRL_SIGNAL_NM ? S->node_n_out[h] : 0, S->edge_in_rank[e], S->edge_out_rank[e2], k) == SIG_RED) {
                     FAIL("I7: step %llu veh %u crossed on red", (unsigned long long)k, i); return -1;
                 }
+                if (check && ctrl == CTRL_STOP && !(S->node_free_from[h] <= k)) {
+                    FAIL("I7: step %llu veh %u crossed a STOP node that was held", (unsigned long long)k, i); return -1;
+                }
+                if (ctrl == CTRL_STOP) {             /* holds the node until it has cleared it */
+                    S->node_free_from[h] = UINT32_MAX;
+                    S->owns_node[i] = 1;
+                }
+                S->made_stop[i] = 0;
                 float xn = S->xt[i] - Cf;
                 xn = fminf(xn, (float)S->edge_len[e2] - 0.0625f);
                 float v0n = S->v0_mult[i] * S->edge_vlim[e2];
+                v0n = fminf(v0n, S->t_vmax[S->veh_type[i]]);
                 list_unlink(S, i, g);
                 S->x[i] = xn; S->v[i] = fminf(S->vt[i], v0n);      /* reading R9 */
                 S->edge[i] = e2; S->lane[i] = (uint8_t)l2; S->r[i]++;
@@ -806,7 +928,7 @@ static int one_step(orc_sim *S, int check, uint64_t order_seed) {
                 S->enter_step[i] = k1;
                 S->relink[S->n_relink++] = i;
                 S->entry_lane[S->n_entry++] = g2;
-                if (S->node_ctrl[h] == CTRL_PRIORITY) S->cross_node[S->n_cross_node++] = h;
+                if (ctrl == CTRL_PRIORITY || ctrl == CTRL_STOP) S->cross_node[S->n_cross_node++] = h;
                 S->cnt.crossings++;
             } else {                                               /* reading R15: held at the line */
                 S->x[i] = Cf - 0.0625f; S->v[i] = 0.0f;
@@ -830,7 +952,7 @@ static int one_step(orc_sim *S, int check, uint64_t order_seed) {
             }
         }
         if (check && S->status[i] == ST_ACTIVE && S->edge[i] == e) {  /* I5 advance bound */
-            double bound = ((double)v_old + 0.5 * S->p.a * S->p.dt) * S->p.dt + 1e-3;
+            double bound = ((double)v_old + 0.5 * S->t_a[S->veh_type[i]] * S->p.dt) * S->p.dt + 1e-3;
             if ((double)S->x[i] - (double)x_old > bound) { FAIL("I5: step %llu veh %u advanced %g > %g", (unsigned long long)k, i, S->x[i] - x_old, bound); return -1; }
         }
     }

@@ -63,6 +63,18 @@ typedef struct orc_params {
     uint32_t insert_clear_cells;
     uint32_t sample_period_steps; /* 0 = no sampling */
     uint32_t emissions;           /* non-zero: per-vehicle CO and fuel accumulators */
+    /* Vehicle types ("a second type of vehicle to represent trucks, to reflect their
+     * differences in size, acceleration, and maximum speed"; reading R31).  n_types == 0: one type
+     * {veh_len, a, no speed cap}.  Otherwise type t = {type_len[t], type_a[t], type_vmax[t]} and
+     * veh_len / a above are not used. */
+    uint32_t n_types;             /* 0..4 */
+    float type_len[4];            /* m */
+    float type_a[4];              /* m/s^2 */
+    float type_vmax[4];           /* m/s; desired speed = min(v0_mult * edge limit, type_vmax) */
+    /* Control variants (readings R34-R36) */
+    uint32_t amber_steps;         /* amber after every green (0 = none) */
+    float stop_dist;              /* CTRL_STOP: a vehicle has made its stop once it is within stop_dist m */
+    float stop_speed;             /*            of the line at no more than stop_speed m/s */
 } orc_params;
 
 /* Work counters: what a byte-scan method would have to touch. */
@@ -85,8 +97,9 @@ typedef struct orc_counters {
 
 typedef struct orc_sim orc_sim;
 
-/* All pointers are host arrays owned by the caller and copied.  v0_mult / mand_dist_m may
- * be NULL.  Returns NULL on invalid input (message in orc_last_error()). */
+/* All pointers are host arrays owned by the caller and copied.  v0_mult / mand_dist_m / veh_type
+ * may be NULL (veh_type: everybody is of type 0).  node_ctrl: 0 FREE, 1 PRIORITY, 2 SIGNAL (one
+ * phase per inbound edge, R16), 3 STOP (R34), 4 SIGNAL_NM (one phase per movement, R35).  Returns NULL on invalid input (message in orc_last_error()). */
 orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
                     const uint32_t *edge_from, const uint32_t *edge_to,
                     const uint32_t *edge_len_m, const uint8_t *edge_lanes,
@@ -95,7 +108,7 @@ orc_sim *orc_create(uint32_t n_nodes, uint32_t n_edges,
                     const uint32_t *sig_offset_steps,
                     uint32_t n_vehicles, const uint64_t *route_off,
                     const uint32_t *route_edges, const float *depart_time_s,
-                    const float *v0_mult, const float *mand_dist_m,
+                    const float *v0_mult, const float *mand_dist_m, const uint8_t *veh_type,
                     const orc_params *params);
 
 /* Advance n steps.  digests (nullable) receives one 64-bit digest per step (state k+1).
@@ -143,6 +156,9 @@ uint8_t orc_speed_code(float v);
 float orc_speed_decode(uint8_t code);
 int orc_signal_green(uint32_t green, uint32_t allred, uint32_t offset, uint32_t n_in,
                      uint32_t in_rank, uint64_t k);
+/* 0 red, 1 green, 2 amber; n_out == 0: one phase per inbound edge, else one per movement. */
+int orc_signal_phase(uint32_t green, uint32_t amber, uint32_t allred, uint32_t offset, uint32_t n_in,
+                     uint32_t n_out, uint32_t in_rank, uint32_t out_rank, uint64_t k);
 uint64_t orc_mix64(uint64_t z);
 
 #ifdef __cplusplus

@@ -310,7 +310,12 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
         phase2(c, S, k, me, dyn_smem, mr_j, n_slots, sample, qr0);
         grid_barrier(c.barrier, target, clk, 2);
         clk.tick(3);
-        if (digests) { phase_digest(c, S, digests + i, me); clk.tick(5); }
+        if (digests) {
+            // the digest reads counters that CTAs already in step i+1 would be bumping (arrivals,
+            // slots handed out): nobody leaves the digest before everybody has finished it
+            phase_digest(c, S, digests + i, me, sh_n_slots[(i + 1) & 1]);
+            grid_barrier(c.barrier, target, clk, 5);
+        }
         if (sort_period && (k + 1) % sort_period == 0) {      // A9 + A10, between two steps
             const uint32_t ns = sort_rank(c, S, me, sh_n_slots[(i + 1) & 1]);
             grid_barrier(c.barrier, target, clk, 4);
@@ -361,7 +366,7 @@ __global__ void __launch_bounds__(256) k_phase2(const __grid_constant__ Ctx c, u
     phase2(c, c.s[cur], k, me, nullptr, 0, sh_n, sample_step(c.p, k), first_queue_rec(c, me));
 }
 __global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, uint32_t cur, unsigned long long* out) {
-    phase_digest(c, c.s[cur], out, who());   // test instrument: may read the slot count per thread
+    phase_digest(c, c.s[cur], out, who(), min(__ldcg(&c.dyn->slot_alloc), c.cap_slots));   // test instrument: may read the slot count per thread
 }
 __global__ void __launch_bounds__(256) k_sort_rank(const __grid_constant__ Ctx c, uint32_t cur) {
     __shared__ uint32_t sh_n;
@@ -766,6 +771,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             const int per_sm_smem = (s->smem_limit - 1024) / s->blocks_per_sm - 1024;
             uint32_t mr_j = (uint32_t)std::max(0, per_sm_smem / (16 * threads));
             const uint32_t grid = (uint32_t)(s->sms * s->blocks_per_sm);
+            if (grid > kMaxCtas) return fail(TS_EINVAL, "step kernel: %u CTAs exceed the %u the sort scratch is sized for", grid, kMaxCtas);
             const uint32_t need_j = (s->L.cap + grid * threads - 1) / (grid * threads);
             mr_j = std::min(mr_j, need_j);
             const size_t smem = (size_t)mr_j * 16 * threads;
@@ -801,8 +807,13 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
                 unsigned long long* dig = d_digests ? d_digests + done : nullptr;
                 const uint32_t parity = s->chunk_no++ & 1u;
                 int rc = launch(k, m, cur, 640, 0u, dig, parity);
-                if (rc) return rc;
-                if ((rc = launch(k, m, cur, 896, 1u, dig, parity))) return rc;
+                if (!rc) rc = launch(k, m, cur, 896, 1u, dig, parity);
+                if (rc) {
+                    // a chunk may have run on the device without the host's step counter following:
+                    // the state is no longer usable until ts_reset
+                    s->sticky = ERR_LOGIC;
+                    return rc;
+                }
                 const uint32_t srt = R ? (k + m) / R - k / R : 0;
                 if (srt & 1) cur ^= 1;
                 k += m; done += m;

@@ -373,8 +373,9 @@ __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k,
 }
 
 // order-independent digest of state k+1 (test instrument, not on the timed path).
-__device__ __forceinline__ void phase_digest(const Ctx& c, const Slots& S, unsigned long long* out, const Who& me) {
-    const uint32_t n_slots = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
+// `n_slots`: the slots of state k+1, read by one thread per CTA after the step's last barrier.
+__device__ __forceinline__ void phase_digest(const Ctx& c, const Slots& S, unsigned long long* out, const Who& me,
+                                             uint32_t n_slots) {
     unsigned long long sum = 0;
     for (uint32_t j = 0;; j++) {
         const uint32_t s = me.slot(j);

@@ -24,6 +24,13 @@ from scipy.sparse.csgraph import connected_components, dijkstra
 SEED_BASE = 180701148  # arxiv id; config n uses SEED_BASE + n (SURVEY.md:476)
 
 CTRL_FREE, CTRL_PRIORITY, CTRL_SIGNAL = 0, 1, 2
+CTRL_STOP, CTRL_SIGNAL_NM = 3, 4     # control variants of PAPER.md:402 (readings R34, R35)
+
+# A second vehicle type "to represent trucks ... size, acceleration, and maximum speed".
+# The paper prints no values; these are this repository's (reading R31): type 0 = car with
+# the BASELINE.json config 1 values, type 1 = truck, 12 m long, half the acceleration, 25 m/s cap.
+TRUCK_PARAMS = dict(n_types=2, type_len=(5.0, 12.0, 0.0, 0.0), type_a=(1.0, 0.5, 0.0, 0.0),
+                    type_vmax=(1000.0, 25.0, 0.0, 0.0), insert_clear_cells=14)
 
 DEFAULT_PARAMS = dict(
     dt=0.5, a=1.0, b=1.5, T=1.5, s0=2.0, veh_len=5.0,            # BASELINE.json config 1
@@ -39,7 +46,7 @@ DEFAULT_PARAMS = dict(
 def make_bundle(name, n_nodes, edge_from, edge_to, edge_len_m, edge_lanes, edge_vlim,
                 node_ctrl, route_off, route_edges, depart_time_s, steps,
                 sig_green_steps=None, sig_allred_steps=None, sig_offset_steps=None,
-                v0_mult=None, mand_dist_m=None, params=None, node_xy=None):
+                v0_mult=None, mand_dist_m=None, params=None, node_xy=None, veh_type=None):
     """Normalise dtypes and fill defaults.  Used by the generators and by hand-made tests."""
     n_nodes = int(n_nodes)
     z = np.zeros(n_nodes, np.uint32)
@@ -67,6 +74,8 @@ def make_bundle(name, n_nodes, edge_from, edge_to, edge_len_m, edge_lanes, edge_
     )
     if node_xy is not None:
         b["node_xy"] = np.asarray(node_xy, np.float64)
+    if veh_type is not None:
+        b["veh_type"] = np.ascontiguousarray(veh_type, np.uint8)
     return b
 
 
@@ -81,6 +90,9 @@ def bundle_sha256(b) -> str:
     for f in _HASH_FIELDS:
         h.update(f.encode())
         h.update(np.ascontiguousarray(b[f]).tobytes())
+    if b.get("veh_type") is not None:
+        h.update(b"veh_type")
+        h.update(np.ascontiguousarray(b["veh_type"]).tobytes())
     h.update(repr(sorted(b["params"].items())).encode())
     return h.hexdigest()
 
@@ -442,9 +454,33 @@ def config3_dense(n_vehicles=1_000_000, steps=2400, workers=None):
                    depart_sd_s=15.0, name="cfg3_dense_diagnostic")
 
 
+def with_trucks(bundle, share=0.10, seed=0, name=None):
+    """The same workload with a share of the vehicles turned into trucks."""
+    rng = np.random.default_rng(SEED_BASE + 100 + seed)
+    ty = (rng.random(bundle["n_vehicles"]) < share).astype(np.uint8)
+    return dict(bundle, name=name or bundle["name"] + "_trucks", veh_type=ty,
+                params=dict(bundle["params"], **TRUCK_PARAMS))
+
+
+def with_controls(bundle, seed=0, amber_steps=6, name=None):
+    """The same workload with the control variants of PAPER.md:402 mixed in: PRIORITY nodes become
+    STOP nodes, half of the SIGNAL nodes get one phase per movement (n*m), every signal an amber."""
+    rng = np.random.default_rng(SEED_BASE + 200 + seed)
+    ctrl = np.array(bundle["node_ctrl"], np.uint8)
+    ctrl[ctrl == CTRL_PRIORITY] = CTRL_STOP
+    sig = np.nonzero(ctrl == CTRL_SIGNAL)[0]
+    ctrl[sig[rng.random(len(sig)) < 0.5]] = CTRL_SIGNAL_NM
+    return dict(bundle, name=name or bundle["name"] + "_controls", node_ctrl=ctrl,
+                params=dict(bundle["params"], amber_steps=amber_steps, stop_dist=4.0, stop_speed=0.5))
+
+
 _BY_NAME = {
     "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5,
     "cfg3_dense": config3_dense,
+    # SURVEY.md 8(f) rows 3 and 4 on config 2's network and demand
+    "cfg2_trucks": lambda: with_trucks(config2()),
+    "cfg2_controls": lambda: with_controls(config2()),
+    "cfg2_trucks_controls": lambda: with_controls(with_trucks(config2())),
     # quick functional checks, not reported workloads
     "cfg3_small": lambda: config3(n_vehicles=50_000, steps=7200, grid=64, n_origin_nodes=512,
                                   depart_mean_s=1200.0, depart_sd_s=400.0, name="cfg3_small"),

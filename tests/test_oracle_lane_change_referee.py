@@ -33,13 +33,15 @@ from test_oracle_pins import _rows, corridor
 EPS = 2e-3
 
 
-def _idm64(p, v, v0, has, s=0.0, dv=0.0):
-    """Eq. 7 in fp64 with readings R1, R2, R8."""
+def _idm64(p, v, v0, has, s=0.0, dv=0.0, a=None):
+    """Eq. 7 in fp64 with readings R1, R2, R8; `a` = the subject vehicle's
+    acceleration ability where vehicle types differ."""
+    a = p["a"] if a is None else a
     free = 1.0 - (v / v0) ** 4
     if not has:
-        return p["a"] * free
-    sstar = p["s0"] + max(0.0, v * p["T"] + v * dv / (2.0 * math.sqrt(p["a"] * p["b"])))
-    return p["a"] * (free - (sstar / max(s, 0.5)) ** 2)
+        return a * free
+    sstar = p["s0"] + max(0.0, v * p["T"] + v * dv / (2.0 * math.sqrt(a * p["b"])))
+    return a * (free - (sstar / max(s, 0.5)) ** 2)
 
 
 def _seen_speed(v):
@@ -51,7 +53,16 @@ def _seen_speed(v):
 class Referee:
     def __init__(self, bundle):
         self.b = bundle
-        self.p = bundle["params"]
+        self.p = p = bundle["params"]
+        # vehicle types: per vehicle its length, acceleration ability and speed cap
+        V = bundle["n_vehicles"]
+        ty = np.zeros(V, int) if bundle.get("veh_type") is None else np.asarray(bundle["veh_type"], int)
+        if p.get("n_types", 0):
+            self.len_of = np.asarray(p["type_len"], float)[ty]
+            self.a_of = np.asarray(p["type_a"], float)[ty]
+            self.vmax_of = np.asarray(p["type_vmax"], float)[ty]
+        else:
+            self.len_of, self.a_of, self.vmax_of = np.full(V, p["veh_len"]), np.full(V, p["a"]), np.full(V, np.inf)
         self.tally = dict(turns=0, accepted=0, skipped=0, polite_flips_to_yes=0, polite_flips_to_no=0,
                           g1_rejects=0, g2_kinematic_rejects=0, g3_rejects=0, mandatory=0, vetoes_of_a_wanted_move=0,
                           discretionary_before_mand_dist=0, with_lag=0, with_lead=0)
@@ -73,7 +84,7 @@ class Referee:
         x, v = float(st["x"][i]), float(st["v"][i])
         C = int(b["edge_len_m"][e])
         n_lanes = int(b["edge_lanes"][e])
-        dt, a, length = p["dt"], p["a"], p["veh_len"]
+        dt, a, length = p["dt"], float(self.a_of[i]), float(self.len_of[i])
         H, Hb = p["lookahead_cells"], p["lookback_cells"]
         margins = []
         if p["lc_period"] == 0 or n_lanes < 2:
@@ -91,7 +102,7 @@ class Referee:
         r = int(st["route_idx"][i])
         last = r == len(route) - 1
         lanes2 = 0 if last else int(b["edge_lanes"][route[r + 1]])
-        v0 = float(np.float32(b["v0_mult"][i]) * np.float32(b["edge_vlim"][e]))
+        v0 = min(float(np.float32(b["v0_mult"][i]) * np.float32(b["edge_vlim"][e])), float(self.vmax_of[i]))
         vlim = float(b["edge_vlim"][e])
         # neighbours in the target lane and the own leader, all on this edge only
         tl = lanes.get((e, lt), [])
@@ -99,15 +110,18 @@ class Referee:
         behind = [(cc, j) for cc, j in tl if max(0, c - Hb) <= cc <= c - 1]
         own = [(cc, j) for cc, j in lanes.get((e, l), []) if c < cc <= min(C - 1, c + H)]
         has_Lt, has_F, lead_on_edge = bool(ahead), bool(behind), bool(own)
-        cLt = vLt = s_Lt = cF = vF = s_lag = 0.0
+        cLt = vLt = s_Lt = cF = vF = s_lag = len_Lt = 0.0
+        a_lag, v0_lag = a, vlim
         if has_Lt:
             cLt, j = ahead[0]
             vLt = _seen_speed(st["v"][j])
-            s_Lt = cLt - length - x
+            len_Lt = float(self.len_of[j])
+            s_Lt = cLt - len_Lt - x                       # the LEADER's length
         if has_F:
             cF, j = behind[-1]
             vF = _seen_speed(st["v"][j])
-            s_lag = x - length - (cF + 1)
+            s_lag = x - length - (cF + 1)                 # the changer's own length
+            a_lag, v0_lag = float(self.a_of[j]), min(vlim, float(self.vmax_of[j]))
         t = self.tally
         t["turns"] += 1
         t["with_lag"] += has_F
@@ -122,14 +136,14 @@ class Referee:
             return l, margins
         aF_new = 0.0
         if has_F:
-            bound = (vF + 0.125 + 0.5 * a * dt) * dt                            # G2 with E4
+            bound = (vF + 0.125 + 0.5 * a_lag * dt) * dt                        # G2 with E4
             ok_s0 = cmp_ge(s_lag, p["s0"])
             ok_kin = cmp_ge(s_lag, bound)
             if not (ok_s0 and ok_kin):
                 if ok_s0:
                     t["g2_kinematic_rejects"] += 1
                 return l, margins
-            aF_new = _idm64(p, vF, vlim, True, s_lag, vF - v)                   # G3
+            aF_new = _idm64(p, vF, v0_lag, True, s_lag, vF - v, a_lag)          # G3
             if not cmp_ge(aF_new, -p["b_safe"]):
                 t["g3_rejects"] += 1
                 return l, margins
@@ -137,13 +151,13 @@ class Referee:
         mand = float(b["mand_dist_m"][i])
         inside = rem <= mand
         margins.append(rem - mand)
-        at_c = _idm64(p, v, v0, has_Lt, s_Lt, v - vLt)
-        a_c = _idm64(p, v, v0, True, own[0][0] - length - x, v - _seen_speed(st["v"][own[0][1]])) if lead_on_edge \
-            else _idm64(p, v, v0, False)
+        at_c = _idm64(p, v, v0, has_Lt, s_Lt, v - vLt, a)
+        a_c = _idm64(p, v, v0, True, own[0][0] - float(self.len_of[own[0][1]]) - x,
+                     v - _seen_speed(st["v"][own[0][1]]), a) if lead_on_edge else _idm64(p, v, v0, False, a=a)
         inc_self = at_c - a_c
         inc = inc_self
         if has_F:
-            a_F = _idm64(p, vF, vlim, has_Lt, cLt - length - (cF + 1), vF - vLt)
+            a_F = _idm64(p, vF, v0_lag, has_Lt, cLt - len_Lt - (cF + 1), vF - vLt, a_lag)
             inc = inc_self + p["politeness"] * (aF_new - a_F)
         if not last and l >= lanes2 and lt < l and inside:
             t["mandatory"] += 1
