@@ -47,7 +47,19 @@ typedef enum ts_status {
 } ts_status;
 
 /* Node control types ("stop and traffic light signals"). */
-enum { TS_CTRL_FREE = 0, TS_CTRL_PRIORITY = 1, TS_CTRL_SIGNAL = 2 };
+/* Controls ("Our system implements stop and traffic light signals"):
+ *  FREE       no control.
+ *  PRIORITY   at most one vehicle crosses the node per step, lowest id first (reading R15).
+ *  SIGNAL     fixed-time light, one phase per inbound edge in round robin (reading R16).
+ *  STOP       "allows just one vehicle at a time into the intersection and waits until the car has
+ *             reached the next edge": every vehicle first comes to a halt at the line (ts_params
+ *             stop_dist / stop_speed), then crosses when the node is free, lowest id first, and
+ *             holds the node until its rear bumper is past it (reading R34).
+ *  SIGNAL_NM  "given an intersection with n inbound edges and m outbound, our system creates the
+ *             geometric combination nm of necessary traffic phasing ... round robin": one phase per
+ *             movement (inbound i, outbound j), number i*m + j, ranks by edge index (reading R35).
+ * Every signal phase is green, then ts_params.amber_steps of amber (R36), then all-red. */
+enum { TS_CTRL_FREE = 0, TS_CTRL_PRIORITY = 1, TS_CTRL_SIGNAL = 2, TS_CTRL_STOP = 3, TS_CTRL_SIGNAL_NM = 4 };
 /* Vehicle status. */
 enum { TS_PENDING = 0, TS_ACTIVE = 1, TS_ARRIVED = 2 };
 
@@ -79,6 +91,8 @@ typedef struct ts_departures {
     const float *v0_mult;             /* [V] desired speed = v0_mult * edge limit; NULL => 1 */
     const float *mand_dist_m;         /* [V] distance to the exit at which a wrong-lane vehicle
                                          turns mandatory; NULL => default */
+    const uint8_t *veh_type;          /* [V] vehicle type < max(1, ts_params.n_types) (PAPER.md:433:
+                                         "a second type of vehicle to represent trucks"); NULL => 0 */
 } ts_departures;
 
 /* Model parameters.  Defaults in DESIGN.md section 3 (BASELINE.json configs 1-2). */
@@ -100,6 +114,20 @@ typedef struct ts_params {
                                     (Eq. 9) totals; costs 8 bytes per vehicle plus 16 per
                                     slot of workspace and 16 coalesced bytes per vehicle-update;
                                     never changes the traffic (see ts_read_emissions) */
+    /* Vehicle types (trucks differ "in size, acceleration, and maximum speed"; DESIGN.md
+     * reading R31).  n_types == 0: one type { veh_len, a, no speed cap }.  Otherwise type t =
+     * { type_len[t] >= 2 m, type_a[t] > 0 m/s^2, type_vmax[t] > 0 m/s } and veh_len / a are not used:
+     * a vehicle's desired speed is min(v0_mult * edge limit, type_vmax), Eq. 7 uses its own `a`,
+     * and every gap is measured to the REAR of the vehicle ahead, i.e. with that vehicle's length
+     * (the atlas carries the occupant's type beside its speed code). */
+    uint32_t n_types;            /* 0..4 */
+    float type_len[4];
+    float type_a[4];
+    float type_vmax[4];
+    /* Control variants (readings R34-R36). */
+    uint32_t amber_steps;        /* amber after every green: a vehicle goes on iff v^2 > 2 b (C - x); 0 = none */
+    float stop_dist;             /* TS_CTRL_STOP: a vehicle has made its stop once it is within stop_dist m of */
+    float stop_speed;            /*   the line at no more than stop_speed m/s (both >= 0) */
 } ts_params;
 
 /* Device resources lent by the caller for the lifetime of the ts_sim. */

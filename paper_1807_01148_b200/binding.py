@@ -35,7 +35,8 @@ class TsRoutes(C.Structure):
 
 
 class TsDepartures(C.Structure):
-    _fields_ = [("depart_time_s", C.c_void_p), ("v0_mult", C.c_void_p), ("mand_dist_m", C.c_void_p)]
+    _fields_ = [("depart_time_s", C.c_void_p), ("v0_mult", C.c_void_p), ("mand_dist_m", C.c_void_p),
+                ("veh_type", C.c_void_p)]
 
 
 class TsParams(C.Structure):
@@ -43,7 +44,14 @@ class TsParams(C.Structure):
                                          "lc_threshold", "mand_dist_default")] + \
                [(n, C.c_uint32) for n in ("lookahead_cells", "lookback_cells", "lc_period",
                                           "entry_zone_cells", "insert_clear_cells", "sample_period_steps",
-                                          "emissions")]
+                                          "emissions", "n_types")] + \
+               [("type_len", C.c_float * 4), ("type_a", C.c_float * 4), ("type_vmax", C.c_float * 4),
+                ("amber_steps", C.c_uint32), ("stop_dist", C.c_float), ("stop_speed", C.c_float)]
+
+
+# ts_params fields a bundle may leave out, with the value that switches the feature off
+_OPTIONAL = dict(emissions=0, n_types=0, type_len=(), type_a=(), type_vmax=(), amber_steps=0,
+                 stop_dist=4.0, stop_speed=0.5)
 
 
 class TsDevice(C.Structure):
@@ -118,13 +126,18 @@ def marshal(bundle):
         "depart_time_s")}
     for k in ("v0_mult", "mand_dist_m"):
         keep[k] = None if b.get(k) is None else np.ascontiguousarray(b[k])
+    keep["veh_type"] = None if b.get("veh_type") is None else np.ascontiguousarray(b["veh_type"], np.uint8)
     net = TsNetwork(int(b["n_nodes"]), int(b["n_edges"]), *[_p(keep[k]) for k in (
         "edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim", "node_ctrl",
         "sig_green_steps", "sig_allred_steps", "sig_offset_steps")])
     routes = TsRoutes(int(b["n_vehicles"]), _p(keep["route_off"]), _p(keep["route_edges"]))
-    dep = TsDepartures(_p(keep["depart_time_s"]), _p(keep["v0_mult"]), _p(keep["mand_dist_m"]))
-    prm = TsParams(**{n: (b["params"].get(n, 0) if n == "emissions" else b["params"][n])
-                      for n, _ in TsParams._fields_})
+    dep = TsDepartures(_p(keep["depart_time_s"]), _p(keep["v0_mult"]), _p(keep["mand_dist_m"]),
+                       _p(keep["veh_type"]))
+    vals = {}
+    for n, ctype in TsParams._fields_:
+        v = b["params"].get(n, _OPTIONAL[n]) if n in _OPTIONAL else b["params"][n]
+        vals[n] = ctype(*[float(x) for x in v]) if n.startswith("type_") else v
+    prm = TsParams(**vals)
     return net, routes, dep, prm, keep
 
 

@@ -75,8 +75,10 @@ struct Layout {
     size_t edges, route_edges, route_begin, queue_rec, dep_rec, codes, occ, queue_state, queue_cand,
         lane_claim, node_claim, dyn, barrier, slots, slots_d, mr_g, cr, rank, hist, base, audit, partial, o_status, o_lane,
         o_edge, o_x, o_v, o_rpos, o_insert, o_arrive, o_cell, o_ridx, st_entered, st_exited,
-        st_exit_steps, st_samp_cnt, st_samp_code, emis, digest;
+        st_exit_steps, st_samp_cnt, st_samp_code, emis, digest, types, edge_aux, edge_from, node_free_from;
     uint32_t emissions = 0;
+    uint32_t ext = 0;          // extended rule set: vehicle types and / or control variants (R31-R36)
+    uint32_t typed = 0;        // more than one vehicle type: the atlas has a type plane
     static constexpr uint32_t kDigestChunk = 8192;
     size_t take(size_t bytes) {
         size_t off = total;
@@ -109,6 +111,9 @@ struct Layout {
         st_samp_code = take((size_t)E * 8);
         emis = take(emissions ? (size_t)V * 8 : 0);      // zeroed by ts_reset with the statistics
         digest = take((size_t)kDigestChunk * 8);
+        types = take(typed ? atlas_chunks * 128 : 0);
+        edge_aux = take(ext ? (size_t)E * 4 : 0); edge_from = take(ext ? (size_t)E * 4 : 0);
+        node_free_from = take(ext ? (size_t)N * 4 : 0);
     }
 };
 
@@ -165,6 +170,10 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_param
     // lane yet holds one reserved slot, which a compaction may drop (then it takes a new one)
     L.cap = (uint32_t)std::min<uint64_t>((uint64_t)L.V + q + 1024ull, 0x7FFFFFF0ull);
     L.emissions = prm->emissions ? 1u : 0u;
+    L.typed = prm->n_types > 1 ? 1u : 0u;
+    L.ext = (prm->n_types != 0 || prm->amber_steps != 0) ? 1u : 0u;
+    for (uint32_t h = 0; h < L.N && !L.ext; h++)
+        if (net->node_ctrl[h] > TS_CTRL_SIGNAL) L.ext = 1u;
     L.plan();
     return TS_OK;
 }
@@ -267,7 +276,7 @@ __device__ __forceinline__ void clock_tick(PhaseClock& clk, int b) { clk.tick(b)
 
 // MAXT = most threads per SM it is launched with: sets the register budget (64 / 80 / 128).
 // EMIS = keep the section 6.3.4 totals (ts_params.emissions).
-template <int MAXT, bool EMIS>
+template <int MAXT, bool EMIS, bool EXT>
 __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ Ctx c, uint32_t k0, uint32_t n,
                                                        uint32_t cur, uint32_t sort_period, uint32_t mr_j,
                                                        unsigned long long* digests, uint32_t profile,
@@ -302,12 +311,12 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
         const uint32_t n_slots = sh_n_slots[i & 1];
         const bool sample = (k == k_sample);
         if (sample) k_sample += sp;
-        phase1<EMIS>(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd, qr0);
+        phase1<EMIS, EXT>(c, S, k, me, dyn_smem, mr_j, n_slots, sample, n_upd, qr0);
         grid_barrier(c.barrier, target, clk, 0);
         clk.tick(1);
         // slots are handed out in phase 1 only: the count the next step works on is final now
         if (me.t == 0) sh_n_slots[(i + 1) & 1] = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
-        phase2(c, S, k, me, dyn_smem, mr_j, n_slots, sample, qr0);
+        phase2<EXT>(c, S, k, me, dyn_smem, mr_j, n_slots, sample, qr0);
         grid_barrier(c.barrier, target, clk, 2);
         clk.tick(3);
         if (digests) {
@@ -344,7 +353,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
 
 // The same phases as separate launches (mode 0: profiling per phase, and a fallback where a
 // cooperative launch is not possible).  Move records go through global memory.
-template <bool EMIS>
+template <bool EMIS, bool EXT>
 __global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
     __shared__ uint32_t red[33];
     uint32_t n_upd = 0;
@@ -353,17 +362,18 @@ __global__ void __launch_bounds__(256) k_phase1(const __grid_constant__ Ctx c, u
     __syncthreads();
     const uint32_t n_slots = sh_n;
     const Who me = who();
-    phase1<EMIS>(c, c.s[cur], k, me, nullptr, 0, n_slots, sample_step(c.p, k), n_upd, first_queue_rec(c, me));
+    phase1<EMIS, EXT>(c, c.s[cur], k, me, nullptr, 0, n_slots, sample_step(c.p, k), n_upd, first_queue_rec(c, me));
     if (blockIdx.x == 0 && threadIdx.x == 0) c.dyn->pad = n_slots;   // phase 2 overwrites dyn->n_slots
     n_upd = block_sum(n_upd, red);
     if (threadIdx.x == 0 && n_upd) atomicAdd(&c.dyn->updates, (unsigned long long)n_upd);
 }
+template <bool EXT>
 __global__ void __launch_bounds__(256) k_phase2(const __grid_constant__ Ctx c, uint32_t k, uint32_t cur) {
     __shared__ uint32_t sh_n;
     if (threadIdx.x == 0) sh_n = __ldcg(&c.dyn->pad);
     __syncthreads();
     const Who me = who();
-    phase2(c, c.s[cur], k, me, nullptr, 0, sh_n, sample_step(c.p, k), first_queue_rec(c, me));
+    phase2<EXT>(c, c.s[cur], k, me, nullptr, 0, sh_n, sample_step(c.p, k), first_queue_rec(c, me));
 }
 __global__ void __launch_bounds__(256) k_digest(const __grid_constant__ Ctx c, uint32_t cur, unsigned long long* out) {
     phase_digest(c, c.s[cur], out, who(), min(__ldcg(&c.dyn->slot_alloc), c.cap_slots));   // test instrument: may read the slot count per thread
@@ -460,16 +470,18 @@ __global__ void k_finish_state(const __grid_constant__ Ctx c, uint32_t* o_cell, 
 
 // The instantiation whose register budget fits `per_sm_threads` resident threads per SM
 // (128 / 96 / 80 / 72 / 64 registers per thread).
-template <bool EMIS>
+template <bool EMIS, bool EXT>
 static const void* step_kernel_of(int per_sm_threads) {
-    if (per_sm_threads <= 512) return (const void*)k_persistent<512, EMIS>;
-    if (per_sm_threads <= 640) return (const void*)k_persistent<640, EMIS>;
-    if (per_sm_threads <= 768) return (const void*)k_persistent<768, EMIS>;
-    if (per_sm_threads <= 896) return (const void*)k_persistent<896, EMIS>;
-    return (const void*)k_persistent<1024, EMIS>;
+    if (per_sm_threads <= 512) return (const void*)k_persistent<512, EMIS, EXT>;
+    if (per_sm_threads <= 640) return (const void*)k_persistent<640, EMIS, EXT>;
+    if (per_sm_threads <= 768) return (const void*)k_persistent<768, EMIS, EXT>;
+    if (per_sm_threads <= 896) return (const void*)k_persistent<896, EMIS, EXT>;
+    return (const void*)k_persistent<1024, EMIS, EXT>;
 }
-static const void* step_kernel(int per_sm_threads, bool emissions) {
-    return emissions ? step_kernel_of<true>(per_sm_threads) : step_kernel_of<false>(per_sm_threads);
+// EXT (vehicle types, control variants) and EMIS (section 6.3.4 totals) are compiled in only where asked for
+static const void* step_kernel(int per_sm_threads, bool emissions, bool ext) {
+    if (ext) return emissions ? step_kernel_of<true, true>(per_sm_threads) : step_kernel_of<false, true>(per_sm_threads);
+    return emissions ? step_kernel_of<true, false>(per_sm_threads) : step_kernel_of<false, false>(per_sm_threads);
 }
 
 // ------------------------------------------------------------------ create / reset
@@ -485,6 +497,17 @@ static int validate(const ts_network* net, const ts_routes* rt, const ts_departu
     if (p->insert_clear_cells < 1 || p->insert_clear_cells > 16)
         return fail(TS_EINVAL, "params: insert_clear_cells must be in 1..16");
     const uint32_t V = rt->n_vehicles, E = net->n_edges, N = net->n_nodes;
+    // vehicle types (reading R31): none given = one type { veh_len, a, no speed cap }
+    if (p->n_types > (uint32_t)kMaxTypes) return fail(TS_EINVAL, "params: n_types must be in 0..%d", kMaxTypes);
+    float max_len = p->n_types ? 0.0f : p->veh_len, max_a = p->n_types ? 0.0f : p->a;
+    for (uint32_t t = 0; t < p->n_types; t++) {
+        if (!(p->type_len[t] >= 2.0f) || !(p->type_a[t] > 0) || !(p->type_vmax[t] > 0))
+            return fail(TS_EINVAL, "params: vehicle type %u needs type_len >= 2, type_a > 0, type_vmax > 0", t);
+        max_len = std::max(max_len, p->type_len[t]); max_a = std::max(max_a, p->type_a[t]);
+    }
+    if (dep->veh_type)
+        for (uint32_t i = 0; i < V; i++)
+            if (dep->veh_type[i] >= std::max(1u, p->n_types)) return fail(TS_EINVAL, "vehicle %u: veh_type %u out of range", i, dep->veh_type[i]);
     float max_mult = 1.0f;
     for (uint32_t i = 0; i < V; i++) {
         if (dep->v0_mult) {
@@ -495,23 +518,41 @@ static int validate(const ts_network* net, const ts_routes* rt, const ts_departu
         if (std::ceil((double)dep->depart_time_s[i] / (double)p->dt) >= 2147483648.0)
             return fail(TS_EINVAL, "vehicle %u: departure step beyond 2^31", i);
     }
+    float max_vlim = 0.0f;
     for (uint32_t e = 0; e < E; e++) {
         if (net->edge_from[e] >= N || net->edge_to[e] >= N) return fail(TS_EINVAL, "edge %u: endpoint out of range", e);
         if (!(net->edge_vlim[e] > 0)) return fail(TS_EINVAL, "edge %u: speed limit must be > 0", e);
+        max_vlim = std::max(max_vlim, net->edge_vlim[e]);
         // a vehicle entering an edge must land short of the zone where lanes may be changed (R14)
-        double adv = (double)net->edge_vlim[e] * max_mult * p->dt + 0.5 * p->a * p->dt * p->dt + p->veh_len;
+        double adv = (double)net->edge_vlim[e] * max_mult * p->dt + 0.5 * max_a * p->dt * p->dt + max_len;
         if (!(adv < (double)p->entry_zone_cells))
             return fail(TS_EINVAL, "edge %u: entry_zone_cells %u too short for the fastest vehicle (%.2f m)", e, p->entry_zone_cells, adv);
     }
-    for (uint32_t h = 0; h < N; h++) {
-        if (net->node_ctrl[h] > 2) return fail(TS_EINVAL, "node %u: unknown control type", h);
-        if (net->node_ctrl[h] == TS_CTRL_SIGNAL) {
-            if (net->sig_green_steps[h] < 1) return fail(TS_EINVAL, "node %u: green must be >= 1 step", h);
-            if ((uint64_t)net->sig_green_steps[h] + net->sig_allred_steps[h] > 65535)
-                return fail(TS_EINVAL, "node %u: green + all-red > 65535 steps", h);
-            if (net->sig_offset_steps[h] >= 0x80000000u) return fail(TS_EINVAL, "node %u: offset >= 2^31", h);
-        }
+    {   // nobody may jump over a leader it never saw: the scans reach further than one step's advance plus a vehicle
+        const double adv = (double)max_vlim * max_mult * p->dt + 0.5 * max_a * p->dt * p->dt + max_len;
+        if (!((double)p->lookahead_cells >= adv))
+            return fail(TS_EINVAL, "params: lookahead_cells %u shorter than one step's advance plus a vehicle length (%.2f m)", p->lookahead_cells, adv);
+        if (p->lc_period != 0 && !((double)p->lookback_cells >= adv))
+            return fail(TS_EINVAL, "params: lookback_cells %u shorter than one step's advance plus a vehicle length (%.2f m)", p->lookback_cells, adv);
     }
+    std::vector<uint32_t> deg_in(N, 0), deg_out(N, 0);
+    for (uint32_t e = 0; e < E; e++) { deg_in[net->edge_to[e]]++; deg_out[net->edge_from[e]]++; }
+    for (uint32_t h = 0; h < N; h++) {
+        const uint32_t ctrl = net->node_ctrl[h];
+        if (ctrl > TS_CTRL_SIGNAL_NM) return fail(TS_EINVAL, "node %u: unknown control type", h);
+        if (ctrl == TS_CTRL_SIGNAL || ctrl == TS_CTRL_SIGNAL_NM) {
+            if (net->sig_green_steps[h] < 1) return fail(TS_EINVAL, "node %u: green must be >= 1 step", h);
+            const uint64_t P = (uint64_t)net->sig_green_steps[h] + p->amber_steps + net->sig_allred_steps[h];
+            if (P > 65535) return fail(TS_EINVAL, "node %u: green + amber + all-red > 65535 steps", h);
+            if (net->sig_offset_steps[h] >= 0x80000000u) return fail(TS_EINVAL, "node %u: offset >= 2^31", h);
+            const uint64_t phases = ctrl == TS_CTRL_SIGNAL_NM ? (uint64_t)deg_in[h] * std::max(1u, deg_out[h]) : deg_in[h];
+            if (deg_in[h] > 255 || deg_out[h] > 255 || phases * P >= (1ull << 24))
+                return fail(TS_EINVAL, "node %u: signal cycle of %llu steps does not fit 24 bits", h, (unsigned long long)(phases * P));
+        }
+        if (ctrl == TS_CTRL_STOP && !(max_len <= 15.0f))
+            return fail(TS_EINVAL, "node %u: STOP control needs vehicle lengths <= 15 m (an edge is >= 16 m)", h);
+    }
+    if (!(p->stop_dist >= 0) || !(p->stop_speed >= 0)) return fail(TS_EINVAL, "params: stop_dist, stop_speed must be >= 0");
     // routes: every entry a valid edge, consecutive edges share a node
     std::atomic<uint32_t> bad_vehicle(0xFFFFFFFFu);
     parallel_chunks(V, [&](size_t b, size_t e_, size_t) {
@@ -550,6 +591,16 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     q.lc_pow2 = (p->lc_period && !(p->lc_period & (p->lc_period - 1))) ? 1u : 0u;
     q.lc_period = p->lc_period; q.insert_clear = p->insert_clear_cells; q.sample_period = p->sample_period_steps;
     q.inv_dt = 1.0f / p->dt;
+    for (int t = 0; t < kMaxTypes; t++) {
+        const bool given = (uint32_t)t < p->n_types;
+        const float len_t = given ? p->type_len[t] : p->veh_len, a_t = given ? p->type_a[t] : p->a;
+        q.t_len[t] = len_t; q.t_a[t] = a_t; q.t_vmax[t] = given ? p->type_vmax[t] : INFINITY;
+        { volatile float ab = a_t * p->b; volatile float r = sqrtf(ab); volatile float K = 2.0f * r; q.t_Kinv[t] = 1.0f / K; }
+        { volatile float h = 0.5f * a_t; q.t_half_a_dt[t] = h * p->dt; }
+        q.t_a_dt[t] = a_t * p->dt;
+    }
+    if (p->n_types) { q.len = q.t_len[0]; q.a = q.t_a[0]; q.Kinv = q.t_Kinv[0]; q.a_dt = q.t_a_dt[0]; q.half_a_dt = q.t_half_a_dt[0]; }
+    q.two_b = 2.0f * p->b; q.stop_dist = p->stop_dist; q.stop_speed = p->stop_speed; q.amber = p->amber_steps;
     c.V = L.V; c.E = L.E; c.N = L.N; c.n_queues = L.Q; c.cap_slots = L.cap; c.sort_groups = L.groups;
     c.edges = at<EdgeRec>(s, L.edges); c.route_edges = at<uint32_t>(s, L.route_edges);
     c.route_begin = at<uint32_t>(s, L.route_begin);
@@ -572,6 +623,10 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     c.st_exit_steps = at<unsigned long long>(s, L.st_exit_steps); c.st_samp_cnt = at<uint32_t>(s, L.st_samp_cnt);
     c.st_samp_code = at<unsigned long long>(s, L.st_samp_code);
     c.emis = L.emissions ? at<float2>(s, L.emis) : nullptr;
+    c.types = L.typed ? at<uint8_t>(s, L.types) : nullptr;
+    c.edge_aux = L.ext ? at<uint32_t>(s, L.edge_aux) : nullptr;
+    c.edge_from = L.ext ? at<uint32_t>(s, L.edge_from) : nullptr;
+    c.node_free_from = L.ext ? at<uint32_t>(s, L.node_free_from) : nullptr;
 }
 
 extern "C" int ts_reset(ts_sim* s) {
@@ -583,6 +638,7 @@ extern "C" int ts_reset(ts_sim* s) {
     CUDA_TRY(cudaMemsetAsync(s->ws + L.node_claim, 0xFF, (size_t)L.N * 8, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.hist, 0, (size_t)L.E * L.groups * 4, st));
     CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.digest - L.st_entered, st));
+    if (L.ext) CUDA_TRY(cudaMemsetAsync(s->ws + L.node_free_from, 0, (size_t)L.N * 4, st));   // every STOP node free
     k_init<<<std::max(1u, std::min(1184u, (L.V + 255) / 256)), 256, 0, st>>>(s->ctx);
     CUDA_TRY(cudaGetLastError());
     s->k = 0; s->cur = 0; s->sticky = 0; s->chunk_no = 0;
@@ -607,9 +663,9 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
 
     const uint32_t V = L.V, E = L.E, N = L.N;
     // per-edge records: atlas row offsets, claim indices, signal plan of the head node
-    std::vector<uint32_t> n_in(N, 0);
+    std::vector<uint32_t> n_in(N, 0), n_out(N, 0);
     std::vector<EdgeRec> edges(E);
-    std::vector<uint8_t> in_rank(E);
+    std::vector<uint8_t> in_rank(E), out_rank(E);
     uint64_t row = 0, lane_base = 0;
     for (uint32_t e = 0; e < E; e++) {
         EdgeRec& r = edges[e];
@@ -620,6 +676,8 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         r.cyc_lc = 1u | ((uint32_t)net->edge_lanes[e] << 24) | (ctrl << 28);
         r.off_sh = 0; r.magic = 1; r.green = 1;          // cycle 1: n mod 1 = 0 < green
         in_rank[e] = (uint8_t)n_in[h]++;
+        if (n_out[net->edge_from[e]] >= 255) return fail(TS_EINVAL, "node %u: more than 255 outbound edges", net->edge_from[e]);
+        out_rank[e] = (uint8_t)n_out[net->edge_from[e]]++;     // rank among the tail node's outbound edges, by edge index
         row += (uint64_t)net->edge_lanes[e] * ((net->edge_len_m[e] + 127) >> 7);
         lane_base += net->edge_lanes[e];
     }
@@ -629,11 +687,15 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     // invariant cycle is done by multiplication on the device (ts_device.cuh).
     for (uint32_t e = 0; e < E; e++) {
         EdgeRec& r = edges[e];
-        if ((r.cyc_lc >> 28) != TS_CTRL_SIGNAL) continue;
+        const uint32_t ctrl_e = r.cyc_lc >> 28;
+        if (ctrl_e != TS_CTRL_SIGNAL && ctrl_e != TS_CTRL_SIGNAL_NM) continue;
         const uint32_t h = r.to_node;
-        const uint64_t P = (uint64_t)net->sig_green_steps[h] + net->sig_allred_steps[h];
-        const uint64_t cycle = (uint64_t)n_in[h] * P;                    // <= 255 * 65535 < 2^24
-        const uint64_t start = (uint64_t)in_rank[e] * P;                 // < cycle
+        // R36: an amber interval after the green; R35: with one phase per movement (i, j), number
+        // i * m + j, the inbound edge's share i * m * P is folded in here and j * P on the device
+        const uint64_t P = (uint64_t)net->sig_green_steps[h] + p->amber_steps + net->sig_allred_steps[h];
+        const uint64_t m_out = ctrl_e == TS_CTRL_SIGNAL_NM ? std::max(1u, n_out[h]) : 1;   // a dead end has one (empty) exit
+        const uint64_t cycle = (uint64_t)n_in[h] * m_out * P;            // < 2^24 (validated)
+        const uint64_t start = (uint64_t)in_rank[e] * m_out * P;         // < cycle
         const uint64_t off = ((uint64_t)net->sig_offset_steps[h] % cycle + cycle - start) % cycle;
         uint32_t l = 0;
         while ((1ull << l) < cycle) l++;
@@ -678,7 +740,8 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         const float v0m = dep->v0_mult ? dep->v0_mult[i] : 1.0f;
         const float md = dep->mand_dist_m ? dep->mand_dist_m[i] : p->mand_dist_default;
         dep_rec[2 * (size_t)n] = make_uint4(i, fbits(v0m), fbits(md), rb);
-        dep_rec[2 * (size_t)n + 1] = make_uint4(rend, rb + 1 < rend ? re[rb + 1] : NONE32, dep_step[i], 0);
+        dep_rec[2 * (size_t)n + 1] = make_uint4(rend, rb + 1 < rend ? re[rb + 1] : NONE32, dep_step[i],
+                                                dep->veh_type ? dep->veh_type[i] : 0u);
     }
     if (queue_rec.size() != L.Q) return fail(TS_EINVAL, "internal: queue count mismatch");
 
@@ -697,6 +760,17 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     chk(up(L.route_begin, route_begin.data(), (size_t)V * 4));
     chk(up(L.queue_rec, queue_rec.data(), (size_t)L.Q * 16));
     chk(up(L.dep_rec, dep_rec.data(), (size_t)V * 32));
+    std::vector<uint32_t> aux;
+    if (L.ext) {
+        aux.resize(E);
+        for (uint32_t e = 0; e < E; e++) {
+            const uint32_t h = net->edge_to[e];
+            const uint64_t P = (uint64_t)net->sig_green_steps[h] + p->amber_steps + net->sig_allred_steps[h];
+            aux[e] = (uint32_t)std::min<uint64_t>(P, 65535) | ((uint32_t)out_rank[e] << 16);
+        }
+        chk(up(L.edge_aux, aux.data(), (size_t)E * 4));
+        chk(up(L.edge_from, net->edge_from, (size_t)E * 4));
+    }
     // the staging vectors die with this scope: make sure the copies have left them
     chk(cudaStreamSynchronize(st));
     if (ce != cudaSuccess) { delete s; return fail(TS_ECUDA, "upload: %s", cudaGetErrorString(ce)); }
@@ -708,7 +782,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     cudaDeviceGetAttribute(&s->l2_bytes, cudaDevAttrL2CacheSize, dev_id);
     bool attr_ok = true;
     for (int t : {512, 640, 768, 896, 1024})
-        attr_ok = attr_ok && cudaFuncSetAttribute(step_kernel(t, s->L.emissions != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) == cudaSuccess;
+        attr_ok = attr_ok && cudaFuncSetAttribute(step_kernel(t, s->L.emissions != 0, s->L.ext != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_limit - 1024) == cudaSuccess;
     if (!attr_ok) {
         delete s;
         return fail(TS_ECUDA, "cannot raise the dynamic shared memory limit of the step kernel");
@@ -775,7 +849,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             const uint32_t need_j = (s->L.cap + grid * threads - 1) / (grid * threads);
             mr_j = std::min(mr_j, need_j);
             const size_t smem = (size_t)mr_j * 16 * threads;
-            const void* kern = step_kernel(threads * s->blocks_per_sm, s->L.emissions != 0);
+            const void* kern = step_kernel(threads * s->blocks_per_sm, s->L.emissions != 0, s->L.ext != 0);
             int per_sm = 0;
             CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
             if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, threads);
@@ -824,9 +898,15 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
         const int g = s->sms * 8, gs = std::min<int>(s->sms * 8, (int)kMaxCtas);
         for (uint32_t i = 0; i < n; i++) {
             const uint32_t k = s->k + i;
-            if (s->L.emissions) k_phase1<true><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
-            else k_phase1<false><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
-            k_phase2<<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            if (s->L.ext) {
+                if (s->L.emissions) k_phase1<true, true><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+                else k_phase1<false, true><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+                k_phase2<true><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            } else {
+                if (s->L.emissions) k_phase1<true, false><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+                else k_phase1<false, false><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+                k_phase2<false><<<g, 256, 0, st>>>(s->ctx, k, s->cur);
+            }
             if (d_digests) k_digest<<<g, 256, 0, st>>>(s->ctx, s->cur, d_digests + i);
             if (R && (k + 1) % R == 0) {
                 k_sort_rank<<<gs, 256, 0, st>>>(s->ctx, s->cur);

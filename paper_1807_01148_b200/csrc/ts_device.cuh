@@ -31,9 +31,14 @@
 namespace ts {
 
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
-enum : uint32_t { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2 };
+// CTRL_STOP: stop control with a persistent node owner (reading R34); CTRL_SIGNAL_NM:
+// one signal phase per movement (inbound edge, outbound edge) ("combination nm"; R35)
+enum : uint32_t { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2, CTRL_STOP = 3, CTRL_SIGNAL_NM = 4 };
 enum : uint32_t { ERR_CELL_CLASH = 1, ERR_SLOTS = 2, ERR_LOGIC = 4 };
-enum : uint32_t { ALIVE = 0x100u };
+// flags in Slots::A.w above the lane number: the vehicle takes part in the steps; has made its stop
+// at the STOP line of its edge; holds the STOP node at the tail of its edge; its type
+enum : uint32_t { ALIVE = 0x100u, STOPPED = 0x200u, OWNS = 0x400u, TYPE_SHIFT = 12, TYPE_MASK = 0x3000u };
+constexpr int kMaxTypes = 4;
 // move-record kinds (uint4.w)
 enum : uint32_t { MR_NONE = 0, MR_MOVE = 1, MR_CLEAR = 2, MR_CROSS = 3 };
 
@@ -86,6 +91,12 @@ struct Params {
     uint32_t lc_period, insert_clear, sample_period;
     uint32_t lc_pow2;      // lc_period is a power of two: the stagger test is a mask
     float inv_dt;          // 1 / dt, rounded once on the host (reading R30)
+    // extended rule set (template parameter EXT of the phases): vehicle types (R31) ...
+    float t_len[kMaxTypes], t_a[kMaxTypes], t_Kinv[kMaxTypes], t_a_dt[kMaxTypes], t_half_a_dt[kMaxTypes], t_vmax[kMaxTypes];
+    // ... and control variants (R34-R36)
+    float two_b;           // 2*b (amber: go on iff v^2 > 2 b (C - x))
+    float stop_dist, stop_speed;
+    uint32_t amber;        // steps of amber after every green
 };
 // a sample is taken with the state after every sample_period-th step.
 __device__ __forceinline__ bool sample_step(const Params& p, uint32_t k) {
@@ -143,6 +154,11 @@ struct Ctx {
     // section 6.3.4 totals, id-ordered { grams of CO, millilitres of fuel }: written when a vehicle
     // arrives and by ts_read_emissions' gather (while it drives they live in Slots::D); nullptr = not kept
     float2* emis;
+    // extended rule set only (nullptr otherwise)
+    uint8_t* types;                     // traffic atlas, type plane: the occupant's vehicle type (valid where occupied)
+    const uint32_t* edge_aux;           // [E] phase length P of the head node's signal | rank among the tail node's outbound edges << 16
+    const uint32_t* edge_from;          // [E] tail node
+    uint32_t* node_free_from;           // [N] CTRL_STOP: first step at which the node is free again (UINT32_MAX while held)
 };
 
 constexpr uint32_t kMaxCtas = 2048;
@@ -187,12 +203,13 @@ __device__ __forceinline__ float idm_free(float v, float v0) {
     float r4 = r2 * r2;
     return 1.0f - r4;
 }
-__device__ __forceinline__ float idm(const Params& p, float v, float v0, bool has, float s, float dv) {
+// `a`, `Kinv`: the subject vehicle's acceleration ability and 1 / (2 sqrt(a b)) (per type).
+__device__ __forceinline__ float idm(const Params& p, float a, float Kinv, float v, float v0, bool has, float s, float dv) {
     float fr = idm_free(v, v0);
-    if (!has) return p.a * fr;
+    if (!has) return a * fr;
     float t = v * p.T;
     float u = v * dv;
-    float w = u * p.Kinv;
+    float w = u * Kinv;
     t = t + w;
     t = fmaxf(t, 0.0f);
     float ss = p.s0 + t;
@@ -200,7 +217,7 @@ __device__ __forceinline__ float idm(const Params& p, float v, float v0, bool ha
     float q = ss / se;
     float q2 = q * q;
     float d = fr - q2;
-    return p.a * d;
+    return a * d;
 }
 
 // Section 6.3.4.  Eq. 8: grams of CO per second at speed v; the paper's v_m is
@@ -223,12 +240,17 @@ __device__ __forceinline__ float fuel_rate(float v, float acc) {
     return 0.666f + 0.072f * dem;
 }
 
-__device__ __forceinline__ bool signal_green(const EdgeRec& e, uint32_t k) {
+// Steps since this inbound edge's (or, with `shift`, this movement's) phase began, modulo the cycle:
+// green while < green, then amber for Params::amber steps, then red.  `shift` < cycle.
+__device__ __forceinline__ uint32_t signal_pos(const EdgeRec& e, uint32_t k, uint32_t shift = 0u) {
     const uint32_t cycle = e.cyc_lc & 0xFFFFFFu;
-    const uint32_t n = k + (e.off_sh & 0xFFFFFFu);        // k < 2^31, off < 2^24
+    const uint32_t n = k + (e.off_sh & 0xFFFFFFu) + shift;   // k < 2^31, off, shift < 2^24
     const uint32_t t = __umulhi(e.magic, n);
     const uint32_t q = (t + ((n - t) >> ((e.off_sh >> 24) & 1u))) >> (e.off_sh >> 25);
-    return n - q * cycle < (uint32_t)e.green;
+    return n - q * cycle;
+}
+__device__ __forceinline__ bool signal_green(const EdgeRec& e, uint32_t k) {
+    return signal_pos(e, k) < (uint32_t)e.green;
 }
 
 // One 256-bit load (sm_100 LDG.256): a record is one 32-byte sector, and a warp whose vehicles sit
@@ -349,6 +371,13 @@ __device__ __forceinline__ void atlas_move(const Ctx& c, uint32_t gc_from, uint3
         else { atomicAnd(occ32 + (gc_from >> 5), ~bf); atomicOr(occ32 + (gc_to >> 5), bt); }
     }
     c.codes[gc_to] = (uint8_t)code;
+}
+// extended rule set: the occupant's type travels with its speed code (`code_type` = code | type << 8)
+__device__ __forceinline__ void atlas_set_type(const Ctx& c, uint32_t gc, uint32_t code_type) {
+    if (c.types) c.types[gc] = (uint8_t)(code_type >> 8);
+}
+__device__ __forceinline__ uint32_t type_at(const uint8_t* types, uint32_t row, int cell) {
+    return __ldcg(types + ((size_t)row << 7) + cell);
 }
 __device__ __forceinline__ void atlas_vacate(const Ctx& c, uint32_t gc) {
     atomicAnd(reinterpret_cast<uint32_t*>(c.occ) + (gc >> 5), ~(1u << (gc & 31)));

@@ -474,6 +474,33 @@ def with_controls(bundle, seed=0, amber_steps=6, name=None):
                 params=dict(bundle["params"], amber_steps=amber_steps, stop_dist=4.0, stop_speed=0.5))
 
 
+# --------------------------------------------------------------------------- re-routing inputs
+
+REROUTE_SHARES = (1.0, 1.0, 0.5, 0.25)     # "all routes the first and second iteration, and
+                                           # then we decay it to half and one-fourth of the vehicles"
+W_UNIT = 256                               # routing weights are integers, 1/256 simulation step (R37)
+
+
+def free_flow_weights(bundle):
+    """The initial routing weights of PAPER.md:386, "estimating the travel time (t_t) of each edge as
+    t_t = sqrt(edge_#lines) edge_length / edge_speed" -- read as length / (speed * sqrt(lanes)), the
+    form under which "most vehicles ... use the highways" as that paragraph goes on to say (DESIGN.md
+    reading R41) -- in the integer units the re-routing call takes.  An INPUT of ts_reroute."""
+    b = bundle
+    t = b["edge_len_m"].astype(np.float64) / (b["edge_vlim"].astype(np.float64) * np.sqrt(b["edge_lanes"].astype(np.float64)))
+    return np.clip(np.rint(t / b["params"]["dt"] * W_UNIT), 1, 1 << 20).astype(np.uint32)
+
+
+def reroute_mask(n_vehicles, iteration, seed=0):
+    """Which vehicles recompute their path in iteration 0, 1, 2, 3: a seeded random
+    subset of the stated share; an INPUT of ts_reroute."""
+    share = REROUTE_SHARES[min(iteration, len(REROUTE_SHARES) - 1)]
+    if share >= 1.0:
+        return np.ones(n_vehicles, np.uint8)
+    rng = np.random.default_rng(SEED_BASE + 300 + 17 * seed + iteration)
+    return (rng.random(n_vehicles) < share).astype(np.uint8)
+
+
 _BY_NAME = {
     "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5,
     "cfg3_dense": config3_dense,
