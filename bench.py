@@ -50,35 +50,51 @@ def load_workload(name):
         raise SystemExit(str(e))
 
 
-def measured_traffic(name, kernel):
-    """DRAM bytes per launch of `kernel` on workload `name` from the committed ncu --set full
-    capture (profiles/r01_kernel_traffic.csv: workload,kernel,dram_read_bytes,dram_write_bytes)."""
-    path = os.path.join(ROOT, "profiles", "r01_kernel_traffic.csv")
+def measured_traffic(name, geometry):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the step kernel over one whole
+    run of workload `name`, from the committed ncu --set full capture of the launch geometry the
+    bench line was measured with (profiles/r02_kernel_traffic.csv:
+    workload,geometry,dram_read_bytes,dram_write_bytes,launches; geometry = "adaptive" -- the default:
+    the sum over the launches of every 2048-step chunk -- or "threadsNNN").  None if that geometry
+    was not captured: a number from another geometry is not this run's traffic."""
+    path = os.path.join(ROOT, "profiles", "r02_kernel_traffic.csv")
     try:
         for line in open(path):
             f = [t.strip() for t in line.split(",")]
-            if len(f) >= 4 and f[0] == name and f[1] == kernel:
+            if len(f) >= 4 and f[0] == name and f[1] == geometry:
                 return float(f[2]) + float(f[3])
     except OSError:
         pass
     return None
 
 
-def bytes_per_update(name):
-    """32 + 8 + scanned cells + 2 (see the comment above); cells from the oracle's counters."""
-    for suffix, what in (("", "full run"), ("_partial", "prefix of the run")):
-        path = os.path.join(ROOT, "tests", "golden", f"trace_{name}{suffix}.json")
+def load_trace(name):
+    for suffix in ("", "_partial"):
         try:
-            t = json.load(open(path))
-            c = t["counters"]
-            cells = (c["own_cells"] + c["next_cells"] + c["lc_cells"]) / c["updates"]
-            if not t.get("complete", True):
-                what = f"first {t['marks'][-1]} of {t['steps']} steps"
-            return 32 + 8 + cells + 2, cells, f"oracle counters, {what}"
-        except (OSError, KeyError, ValueError, ZeroDivisionError):
+            return json.load(open(os.path.join(ROOT, "tests", "golden", f"trace_{name}{suffix}.json")))
+        except (OSError, ValueError):
             continue
-    cells = SCAN_CELLS_FALLBACK.get(name.replace("_small", ""), 60.0)
-    return 32 + 8 + cells + 2, cells, "estimate"
+    return None
+
+
+def bytes_per_update(name):
+    """32 + 8 + scanned cells + 2 (see the comment above); cells from the oracle's counters.
+    Returns (bytes, cells, source, bytes with every scan rounded up to 16-cell pieces, its source)."""
+    t = load_trace(name)
+    try:
+        c = t["counters"]
+        cells = (c["own_cells"] + c["next_cells"] + c["lc_cells"]) / c["updates"]
+        what = "full run" if t.get("complete", True) else f"first {t['marks'][-1]} of {t['steps']} steps"
+        if "own_chunks16" in c:
+            cells16 = 16.0 * (c["own_chunks16"] + c["next_chunks16"] + c["lc_chunks16"]) / c["updates"]
+            src16 = "oracle counters (every scan rounded up to 16 cells)"
+        else:       # trace written before the oracle counted pieces: half a piece per scan on average
+            scans = (c["updates"] + 2 * c["lc_evals"]) / c["updates"] + min(1.0, c["next_cells"] / max(1, c["own_cells"]))
+            cells16, src16 = cells + 7.5 * scans, "estimate: raw cells + 7.5 per scan"
+        return 32 + 8 + cells + 2, cells, f"oracle counters, {what}", 32 + 8 + cells16 + 2, src16
+    except (TypeError, KeyError, ZeroDivisionError):
+        cells = SCAN_CELLS_FALLBACK.get(name.replace("_small", ""), 60.0)
+        return 32 + 8 + cells + 2, cells, "estimate", 32 + 8 + cells + 7.5 + 2, "estimate"
 
 
 class ClockSampler:
@@ -144,6 +160,17 @@ def time_oracle(bundle, budget_s, chunk=600):
     return upd, dt, steps
 
 
+def whole_run_baseline(name):
+    """The oracle's rate over the WHOLE run of the config, from the stored trace's wall time (written
+    by tests/golden/make_golden.py on the build machine, not on this box): context for the prefix
+    sample timed here, which covers only the free-flowing start of the run."""
+    t = load_trace(name)
+    if not t or not t.get("seconds") or not t.get("complete", True):
+        return {"whole_run_value": None}
+    return {"whole_run_value": t["counters"]["updates"] / t["seconds"], "whole_run_threads": t.get("threads", 1),
+            "whole_run_note": "stored trace (tests/golden), oracle wall time on the machine that wrote it"}
+
+
 def whole_job(total_ms_local, units_per_rank, dist=None, device="cpu"):
     """Replicas only: every rank ran the same number of units; the job's time
     is the MAX over ranks, its work the sum.  Returns (units/s of the whole job, max ms)."""
@@ -175,7 +202,8 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "config": {"workload": bundle["name"], "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": dict({"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                              "box_cores": os.cpu_count()}, **whole_run_baseline(args.workload)),
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -200,6 +228,7 @@ def main():
                     help="keep the per-vehicle CO / fuel totals of PAPER.md:408-423 (SURVEY.md 8(f) row 2) during the run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end leg (profiling runs)")
+    ap.add_argument("--no-window", action="store_true", help="skip the busiest-window pass (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -282,6 +311,22 @@ def main():
         "sig_allred_steps", "sig_offset_steps", "route_off", "route_edges", "depart_time_s", "v0_mult", "mand_dist_m"))
     V = bundle["n_vehicles"]
     d2h = V * (1 + 4 + 1 + 4 + 4 + 4 + 4 + 4 + 4) + 64
+    # the rate over the 3600-step window with the most active vehicles, beside the whole run
+    window = None
+    if rank == 0 and not args.start_step and sim_steps > 3600 and not args.no_window:
+        sim.reset()
+        prev, best = 0, None
+        for w0 in range(0, sim_steps, 3600):
+            n = min(3600, sim_steps - w0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); sim.step(n); e1.record(stream)
+            tot = int(sim.read_counts()["vehicle_updates"])
+            if n == 3600 and (best is None or tot - prev > best[1]):
+                best = (w0, tot - prev, e0.elapsed_time(e1))
+            prev = tot
+        if best:
+            window = {"first_step": best[0], "steps": 3600, "vehicle_updates": best[1], "mean_active": best[1] / 3600,
+                      "value": best[1] / (best[2] / 1e3), "unit": UNIT, "us_per_sim_step": 1e3 * best[2] / 3600}
     sim.close()
     del sim
     pinned = dict(bundle)
@@ -317,7 +362,7 @@ def main():
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    bpu, cells, bsrc = bytes_per_update(args.workload)
+    bpu, cells, bsrc, bpu16, bsrc16 = bytes_per_update(args.workload)
     launch_s = (sum(ms) / len(ms)) / 1e3                  # one k_persistent launch per bench step
     achieved = bpu * updates / launch_s / 1e9
     # mode 1: one cooperative launch per ts_step call, or -- adaptive CTA size, the default when no
@@ -325,6 +370,11 @@ def main():
     adaptive = args.mode == 1 and not (args.threads or args.blocks_per_sm or args.profile)
     launches_per_run = (2 * sim_steps if args.mode != 1 else
                         2 * ((sim_steps + 2047) // 2048) if adaptive else 1)
+    geometry = "adaptive" if adaptive else f"threads{args.threads or 640}"
+    traffic = (measured_traffic(args.workload, geometry)
+               if args.mode == 1 and not args.start_step and not args.sim_steps and not args.emissions else None)
+    traffic_src = (f"ncu --set full, geometry {geometry}, whole run (profiles/r02_kernel_traffic.csv)" if traffic is not None
+                   else f"no ncu capture of geometry {geometry} for this workload")
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
@@ -342,8 +392,11 @@ def main():
         "gpu_launches": args.steps * launches_per_run,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak,
-                     "traffic": measured_traffic(args.workload, "k_persistent") if args.mode == 1 and not args.start_step and not args.sim_steps else None,
+                     "frac": achieved / peak, "frac_nominal": achieved / 8000.0, "peak_nominal": 8000.0,
+                     "traffic": traffic, "traffic_source": traffic_src,
+                     "bytes_per_update_chunk16": bpu16, "achieved_chunk16": bpu16 * updates / launch_s / 1e9,
+                     "frac_chunk16": bpu16 * updates / launch_s / 1e9 / peak, "chunk16_source": bsrc16,
+                     "busiest_window": window,
                      "peak_source": peak_src,
                      "kernel": "k_persistent" if args.mode == 1 else "k_phase1+k_phase2",
                      "bytes_per_update": bpu, "scan_cells_per_update": cells, "bytes_source": bsrc,
@@ -352,8 +405,11 @@ def main():
     if not args.no_cpu_baseline:
         upd, dt, steps = time_oracle(bundle, 15.0)
         out["cpu_baseline"] = {"value": upd / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                               "box_cores": os.cpu_count(),
                                "sample": f"first {steps} of {bundle['steps']} simulation steps of {bundle['name']} "
-                                         f"({upd} vehicle-updates, {dt:.1f} s, single thread)"}
+                                         f"({upd} vehicle-updates, {dt:.1f} s, single thread): the free-flowing "
+                                         "start of the run, where the oracle is fastest"}
+        out["cpu_baseline"].update(whole_run_baseline(args.workload))
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

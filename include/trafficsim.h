@@ -128,6 +128,11 @@ typedef struct ts_params {
     uint32_t amber_steps;        /* amber after every green: a vehicle goes on iff v^2 > 2 b (C - x); 0 = none */
     float stop_dist;             /* TS_CTRL_STOP: a vehicle has made its stop once it is within stop_dist m of */
     float stop_speed;            /*   the line at no more than stop_speed m/s (both >= 0) */
+    /* Re-routing (ts_reroute): route entries to reserve for each of the two route
+     * tables (>= the entries of the routes given; new routes may be longer).  0 = ts_reroute is not
+     * available and no workspace is spent on it (one shortest-path tree of N words per distinct
+     * origin node, the graph in CSR form, 148 trees in flight). */
+    uint32_t route_capacity;
 } ts_params;
 
 /* Device resources lent by the caller for the lifetime of the ts_sim. */
@@ -201,6 +206,40 @@ int ts_read_edge_stats(ts_sim *sim, ts_edge_stats_out *out, int reset);
  * the fp32 sums are reproducible bit for bit.  Synchronises.  TS_EINVAL unless the sim was
  * created with ts_params.emissions != 0. */
 int ts_read_emissions(ts_sim *sim, float *co_g, float *fuel_ml);
+
+/* Iterative decaying re-routing, PAPER.md:386 (section 6.3.1: "we use the microsimulation measurements
+ * to update those weights and repeat the microsimulation ... we recompute all routes the first and second
+ * iteration, and then we decay it to half and one-fourth of the vehicles") with PAPER.md:431 ("we replace
+ * [per-vehicle Dijkstra] with ... All Pairs Shortest Path"): one shortest-path tree per distinct origin.
+ * Readings R37-R41 of DESIGN.md:
+ *   weights   w[e] = round-half-up(256 * exit_steps_sum[e] / exited[e]) from the statistics accumulated
+ *             since the last reset (what ts_read_edge_stats shows), or w_free[e] where no vehicle has
+ *             left the edge; clamped to 1..2^20; units of 1/256 simulation step; all integer.
+ *   w_free    HOST array [E], 1..2^20: the caller's free-flow weights (the paper's initialisation).
+ *   mask      HOST array [V] or NULL (= everybody): vehicles with mask[i] != 0 get the shortest path
+ *             from the tail node of their first edge to the head node of their last edge, ties broken
+ *             by taking at every node, walking back from the destination, the inbound edge with the
+ *             smallest (distance, edge id); the others keep their route; so does a vehicle whose
+ *             origin is its destination.
+ * All on the device (weights, trees, route extraction, offsets); the host only rebuilds the index of
+ * departure queues for the new first edges.  Ends with ts_reset: step 0, statistics cleared.
+ * out (nullable) receives counts, device times and, if out->w != NULL, the E weights used (host pointer
+ * unless ts_device.out_on_device).  Synchronises.
+ * Errors: TS_EINVAL (route_capacity == 0, bad w_free, a path cost beyond 2^32), TS_ENOMEM (new routes
+ * longer than route_capacity; the routes in use are then unchanged). */
+typedef struct ts_reroute_out {
+    uint32_t n_rerouted;      /* vehicles asked to re-route */
+    uint32_t n_trees;         /* shortest-path trees computed */
+    uint64_t route_entries;   /* length of the new route table */
+    float sssp_ms;            /* device time of the tree kernel */
+    float device_ms;          /* device time of weights + trees + extraction */
+    uint32_t *w;              /* [E] or NULL */
+} ts_reroute_out;
+int ts_reroute(ts_sim *sim, const uint32_t *w_free, const uint8_t *mask, ts_reroute_out *out);
+
+/* The routes in use: HOST arrays route_off [V+1] and route_edges [*n_entries] (either may be NULL;
+ * call once with both NULL to learn *n_entries).  Synchronises. */
+int ts_read_routes(ts_sim *sim, uint64_t *route_off, uint32_t *route_edges, uint64_t *n_entries);
 
 /* Tuning knobs that never change results.
  *  "mode"          1 (default) = ts_step(n) is ONE persistent cooperative kernel looping over

@@ -35,7 +35,7 @@ class OrcParams(C.Structure):
 
 _COUNTER_NAMES = ["updates", "own_cells", "next_cells", "lc_evals", "lc_cells", "lc_accepts",
                   "lc_mandatory", "crossings", "cross_lost", "held_red", "cap_bound",
-                  "departures", "arrivals", "peak_active"]
+                  "departures", "arrivals", "peak_active", "own_chunks16", "next_chunks16", "lc_chunks16"]
 
 
 class OrcCounters(C.Structure):

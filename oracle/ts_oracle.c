@@ -520,9 +520,9 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
             s_lead = (float)cL - S->t_len[S->veh_type[j]];   /* E3 same edge: the LEADER's length */
             s_lead = s_lead - x;
             dv_lead = v - orc_speed_decode(orc_speed_code(S->v[j]));
-            cnt->own_cells += (uint64_t)(cL - c);
+            cnt->own_cells += (uint64_t)(cL - c); cnt->own_chunks16 += (uint64_t)(cL - c + 15) / 16;
         } else {
-            cnt->own_cells += (uint64_t)(lim - c);
+            cnt->own_cells += (uint64_t)(lim - c); cnt->own_chunks16 += (uint64_t)(lim - c + 15) / 16;
             int32_t Hp = H - (C - 1 - c);
             if (!last && may_cross && Hp > 0) {
                 int32_t C2 = (int32_t)S->edge_len[e2];
@@ -535,9 +535,9 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
                     s_lead = s_lead + (float)cL2;
                     s_lead = s_lead - S->t_len[S->veh_type[j2]];
                     dv_lead = v - orc_speed_decode(orc_speed_code(S->v[j2]));
-                    cnt->next_cells += (uint64_t)(cL2 + 1);
+                    cnt->next_cells += (uint64_t)(cL2 + 1); cnt->next_chunks16 += (uint64_t)(cL2 + 1 + 15) / 16;
                 } else {
-                    cnt->next_cells += (uint64_t)(lim2 + 1);
+                    cnt->next_cells += (uint64_t)(lim2 + 1); cnt->next_chunks16 += (uint64_t)(lim2 + 1 + 15) / 16;
                 }
             }
         }
@@ -572,16 +572,16 @@ static void vehicle_intent(orc_sim *S, uint32_t i, orc_counters *cnt) {
                 len_Lt = S->t_len[S->veh_type[jl]];
                 s_Lt = (float)cLt - len_Lt;
                 s_Lt = s_Lt - x;
-                cnt->lc_cells += (uint64_t)(cLt - c + 1);
-            } else cnt->lc_cells += (uint64_t)(lim - c + 1);
+                cnt->lc_cells += (uint64_t)(cLt - c + 1); cnt->lc_chunks16 += (uint64_t)(cLt - c + 1 + 15) / 16;
+            } else { cnt->lc_cells += (uint64_t)(lim - c + 1); cnt->lc_chunks16 += (uint64_t)(lim - c + 1 + 15) / 16; }
             if (jf != NONE && cell_of(S, (uint32_t)jf) >= lo) {
                 has_F = 1; cF = cell_of(S, (uint32_t)jf);
                 tyF = S->veh_type[jf];
                 vF = orc_speed_decode(orc_speed_code(S->v[jf]));
                 s_lag = x - len;                /* E3 lag */
                 s_lag = s_lag - (float)(cF + 1);
-                cnt->lc_cells += (uint64_t)(c - cF);
-            } else cnt->lc_cells += (uint64_t)(c - lo);
+                cnt->lc_cells += (uint64_t)(c - cF); cnt->lc_chunks16 += (uint64_t)(c - cF + 15) / 16;
+            } else { cnt->lc_cells += (uint64_t)(c - lo); cnt->lc_chunks16 += (uint64_t)(c - lo + 15) / 16; }
 
             int ok = 1;
             float aF_new = 0.0f;

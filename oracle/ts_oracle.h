@@ -93,6 +93,9 @@ typedef struct orc_counters {
     uint64_t departures;
     uint64_t arrivals;
     uint64_t peak_active;
+    /* the same scans counted in 16-cell pieces (a scan of n cells touches ceil(n/16) of them):
+     * SURVEY.md 8(d) asks for the algorithmic bytes "rounded up to 16-cell chunks" beside the raw cells */
+    uint64_t own_chunks16, next_chunks16, lc_chunks16;
 } orc_counters;
 
 typedef struct orc_sim orc_sim;

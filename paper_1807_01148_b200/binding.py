@@ -17,7 +17,7 @@ TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
            "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile",
-           "ts_read_emissions", "ts_destroy", "ts_last_error", "ts_version"]
+           "ts_read_emissions", "ts_reroute", "ts_read_routes", "ts_destroy", "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -46,12 +46,13 @@ class TsParams(C.Structure):
                                           "entry_zone_cells", "insert_clear_cells", "sample_period_steps",
                                           "emissions", "n_types")] + \
                [("type_len", C.c_float * 4), ("type_a", C.c_float * 4), ("type_vmax", C.c_float * 4),
-                ("amber_steps", C.c_uint32), ("stop_dist", C.c_float), ("stop_speed", C.c_float)]
+                ("amber_steps", C.c_uint32), ("stop_dist", C.c_float), ("stop_speed", C.c_float),
+                ("route_capacity", C.c_uint32)]
 
 
 # ts_params fields a bundle may leave out, with the value that switches the feature off
 _OPTIONAL = dict(emissions=0, n_types=0, type_len=(), type_a=(), type_vmax=(), amber_steps=0,
-                 stop_dist=4.0, stop_speed=0.5)
+                 stop_dist=4.0, stop_speed=0.5, route_capacity=0)
 
 
 class TsDevice(C.Structure):
@@ -69,6 +70,11 @@ class TsStateOut(C.Structure):
 class TsEdgeStatsOut(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("entered", "exited", "exit_steps_sum", "sample_count_sum",
                                           "sample_speedcode_sum")] + [("n_samples", C.c_uint32)]
+
+
+class TsRerouteOut(C.Structure):
+    _fields_ = [("n_rerouted", C.c_uint32), ("n_trees", C.c_uint32), ("route_entries", C.c_uint64),
+                ("sssp_ms", C.c_float), ("device_ms", C.c_float), ("w", C.c_void_p)]
 
 
 class TsError(RuntimeError):
@@ -98,11 +104,13 @@ def load():
         L.ts_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
         L.ts_read_profile.argtypes = [C.c_void_p, C.c_void_p]
         L.ts_read_emissions.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.ts_reroute.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.ts_read_routes.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]
         L.ts_destroy.argtypes = [C.c_void_p]
         L.ts_destroy.restype = None
         L.ts_last_error.restype = C.c_char_p
         L.ts_version.restype = C.c_char_p
-        for n in EXPORTS[:10]:
+        for n in EXPORTS[:12]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -195,6 +203,26 @@ class Sim:
         out.update(step=o.step, n_pending=o.n_pending, n_active=o.n_active, n_arrived=o.n_arrived,
                    vehicle_updates=o.vehicle_updates)
         return out
+
+    def reroute(self, w_free, mask=None):
+        """ts_reroute: new routes for the masked vehicles from the edge statistics accumulated so far
+        (PAPER.md:386); resets the simulation.  Returns counts, device times and the weights used."""
+        w_free = np.ascontiguousarray(w_free, np.uint32)
+        m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+        w = np.zeros(self.E, np.uint32)
+        o = TsRerouteOut(w=w.ctypes.data)
+        _check(load().ts_reroute(self._h, w_free.ctypes.data, None if m is None else m.ctypes.data, C.byref(o)))
+        return dict(n_rerouted=o.n_rerouted, n_trees=o.n_trees, route_entries=o.route_entries,
+                    sssp_ms=o.sssp_ms, device_ms=o.device_ms, w=w)
+
+    def read_routes(self):
+        """ts_read_routes: (route_off [V+1] uint64, route_edges uint32) of the routes in use."""
+        n = C.c_uint64()
+        _check(load().ts_read_routes(self._h, None, None, C.byref(n)))
+        off = np.zeros(self.V + 1, np.uint64)
+        edges = np.zeros(int(n.value), np.uint32)
+        _check(load().ts_read_routes(self._h, off.ctypes.data, edges.ctypes.data, C.byref(n)))
+        return off, edges
 
     def read_counts(self):
         """Scalars only (no per-vehicle arrays are copied)."""

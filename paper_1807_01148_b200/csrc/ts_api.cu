@@ -22,6 +22,7 @@
 #include "../../include/trafficsim.h"
 #include "ts_phases.cuh"
 #include "ts_sort.cuh"
+#include "ts_reroute.cuh"
 
 namespace cg = cooperative_groups;
 using namespace ts;
@@ -79,6 +80,13 @@ struct Layout {
     uint32_t emissions = 0;
     uint32_t ext = 0;          // extended rule set: vehicle types and / or control variants (R31-R36)
     uint32_t typed = 0;        // more than one vehicle type: the atlas has a type plane
+    // re-routing (ts_params.route_capacity != 0): a second route table, the graph in CSR form, one
+    // shortest-path tree per distinct origin node, per-vehicle origin / destination / new offsets
+    uint64_t Rcap = 0;         // entries per route table
+    uint32_t n_src = 0, Qcap = 0;
+    size_t rr_routes2, rr_end, rr_origin, rr_dest, rr_srcidx, rr_mask, rr_newlen, rr_newoff, rr_bsum, rr_first2,
+        rr_out_off, rr_out_edge, rr_efrom, rr_eto, rr_w, rr_wfree, rr_src, rr_todo, rr_pred, rr_lab, rr_fa, rr_fb,
+        rr_stamp, rr_err;
     static constexpr uint32_t kDigestChunk = 8192;
     size_t take(size_t bytes) {
         size_t off = total;
@@ -86,8 +94,9 @@ struct Layout {
         return off;
     }
     void plan() {
+        const size_t Q = std::max(this->Q, Qcap);        // re-routing may open queues on other edges
         edges = take((size_t)E * sizeof(EdgeRec));
-        route_edges = take(R * 4);
+        route_edges = take(std::max<uint64_t>(R, Rcap) * 4);
         route_begin = take((size_t)V * 4);
         queue_rec = take((size_t)Q * 16);
         dep_rec = take((size_t)V * 32);
@@ -114,6 +123,18 @@ struct Layout {
         types = take(typed ? atlas_chunks * 128 : 0);
         edge_aux = take(ext ? (size_t)E * 4 : 0); edge_from = take(ext ? (size_t)E * 4 : 0);
         node_free_from = take(ext ? (size_t)N * 4 : 0);
+        if (Rcap) {
+            rr_routes2 = take(Rcap * 4); rr_end = take((size_t)V * 4);
+            rr_origin = take((size_t)V * 4); rr_dest = take((size_t)V * 4); rr_srcidx = take((size_t)V * 4);
+            rr_mask = take(V); rr_newlen = take(((size_t)V + 1) * 4); rr_newoff = take(((size_t)V + 1) * 4);
+            rr_bsum = take(((size_t)V / (kScanBlock * kScanItems) + 2) * 4); rr_first2 = take((size_t)V * 8);
+            rr_out_off = take(((size_t)N + 1) * 4); rr_out_edge = take((size_t)E * 4);
+            rr_efrom = take((size_t)E * 4); rr_eto = take((size_t)E * 4); rr_w = take((size_t)E * 4); rr_wfree = take((size_t)E * 4);
+            rr_src = take((size_t)n_src * 4); rr_todo = take((size_t)n_src * 4);
+            rr_pred = take((size_t)n_src * N * 4);
+            rr_lab = take((size_t)kRrCtas * N * 8); rr_fa = take((size_t)kRrCtas * N * 4); rr_fb = take((size_t)kRrCtas * N * 4);
+            rr_stamp = take((size_t)kRrCtas * N * 4); rr_err = take(4);
+        }
     }
 };
 
@@ -166,9 +187,23 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_param
     for (uint32_t i = 0; i < L.V; i++)
         if (!is_origin[fe[i]]) { is_origin[fe[i]] = 1; q++; }
     L.Q = q;
+    if (prm->route_capacity) {
+        // re-routed vehicles keep their origin NODE: a new route may start on any of its outbound edges
+        if (prm->route_capacity < L.R) return fail(TS_EINVAL, "params: route_capacity %u below the %llu entries of the routes given", prm->route_capacity, (unsigned long long)L.R);
+        L.Rcap = prm->route_capacity;
+        std::vector<uint8_t> is_src(L.N, 0);
+        std::vector<uint32_t> deg(L.N, 0);
+        for (uint32_t e = 0; e < L.E; e++) if (net->edge_from[e] < L.N) deg[net->edge_from[e]]++;
+        uint64_t qcap = 0;
+        for (uint32_t i = 0; i < L.V; i++) {
+            const uint32_t o = net->edge_from[fe[i]];
+            if (o < L.N && !is_src[o]) { is_src[o] = 1; L.n_src++; qcap += deg[o]; }
+        }
+        L.Qcap = (uint32_t)std::min<uint64_t>(qcap, L.E);
+    }
     // a vehicle takes one slot when it departs; a queue head that is ready but has not won its
     // lane yet holds one reserved slot, which a compaction may drop (then it takes a new one)
-    L.cap = (uint32_t)std::min<uint64_t>((uint64_t)L.V + q + 1024ull, 0x7FFFFFF0ull);
+    L.cap = (uint32_t)std::min<uint64_t>((uint64_t)L.V + std::max(q, L.Qcap) + 1024ull, 0x7FFFFFF0ull);
     L.emissions = prm->emissions ? 1u : 0u;
     L.typed = prm->n_types > 1 ? 1u : 0u;
     L.ext = (prm->n_types != 0 || prm->amber_steps != 0) ? 1u : 0u;
@@ -212,6 +247,11 @@ struct ts_sim {
     int smem_limit = 0;
     int l2_bytes = 0;
     uint32_t sticky = 0;
+    // re-routing: what the host needs to rebuild the departure-queue index for new routes
+    std::vector<EdgeRec> edges_h;
+    std::vector<uint32_t> dep_step_h, v0m_bits_h, mand_bits_h, type_h, src_idx_h, first_h;
+    uint32_t route_cur = 0;   // which route table is in use
+    RrCtx rr;
 };
 
 template <typename T>
@@ -486,6 +526,42 @@ static const void* step_kernel(int per_sm_threads, bool emissions, bool ext) {
 
 // ------------------------------------------------------------------ create / reset
 
+// Departure queues (R19): one per distinct first edge, FIFO by (departure step, id).  One 32-byte
+// departure record per vehicle in queue order { id, v0_mult, mand, route begin } { route end, second
+// edge, departure step, type } and one 16-byte record per queue { row of lane 0, lane_base, end, edge }.
+// Used by ts_create and, for the new first edges, by ts_reroute.
+static void build_queues(uint32_t V, uint32_t E, const std::vector<EdgeRec>& edges, const uint32_t* first,
+                         const uint32_t* second, const uint32_t* rbegin, const uint32_t* rend,
+                         const uint32_t* dep_step, const uint32_t* v0m_bits, const uint32_t* mand_bits,
+                         const uint32_t* type, std::vector<uint4>& dep_rec, std::vector<uint4>& queue_rec) {
+    // counting sort by first edge (ids stay ascending inside an edge), then each queue by
+    // departure step, stable -- i.e. by (edge, departure step, id) -- queues in parallel
+    std::vector<uint32_t> order(V), q_begin((size_t)E + 1, 0);
+    for (uint32_t i = 0; i < V; i++) q_begin[first[i] + 1]++;
+    for (uint32_t e = 0; e < E; e++) q_begin[e + 1] += q_begin[e];
+    {
+        std::vector<uint32_t> fill(q_begin.begin(), q_begin.end() - 1);
+        for (uint32_t i = 0; i < V; i++) order[fill[first[i]]++] = i;
+    }
+    parallel_chunks(E, [&](size_t b, size_t e_, size_t) {
+        for (size_t e = b; e < e_; e++)
+            if (q_begin[e + 1] - q_begin[e] > 1)
+                std::stable_sort(order.begin() + q_begin[e], order.begin() + q_begin[e + 1],
+                                 [&](uint32_t x, uint32_t y) { return dep_step[x] < dep_step[y]; });
+    });
+    dep_rec.assign(2 * (size_t)V, make_uint4(0, 0, 0, 0));
+    queue_rec.clear();
+    for (uint32_t n = 0; n < V; n++) {
+        const uint32_t i = order[n], e = first[i];
+        if (n == 0 || e != queue_rec.back().w) {
+            if (!queue_rec.empty()) queue_rec.back().z = n;
+            queue_rec.push_back(make_uint4(edges[e].row, edges[e].lane_base, V, e));
+        }
+        dep_rec[2 * (size_t)n] = make_uint4(i, v0m_bits[i], mand_bits[i], rbegin[i]);
+        dep_rec[2 * (size_t)n + 1] = make_uint4(rend[i], second[i], dep_step[i], type[i]);
+    }
+}
+
 static int validate(const ts_network* net, const ts_routes* rt, const ts_departures* dep, const ts_params* p) {
     if (!dep || !p || !dep->depart_time_s) return fail(TS_EINVAL, "null argument");
     if (!(p->dt > 0) || !(p->a > 0) || !(p->b > 0) || !(p->T >= 0) || !(p->s0 >= 0))
@@ -706,43 +782,25 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         r.green = (uint16_t)net->sig_green_steps[h];
     }
     // departure queues: per first edge, FIFO by (departure step, id) (R19)
-    std::vector<uint32_t> dep_step(V), route_begin(V), order(V);
+    std::vector<uint32_t> dep_step(V), route_begin(V);
     for (uint32_t i = 0; i < V; i++) {
         dep_step[i] = (uint32_t)std::ceil((double)dep->depart_time_s[i] / (double)p->dt);
         route_begin[i] = (uint32_t)rt->route_off[i];
     }
-    // counting sort by first edge (ids stay ascending inside an edge), then each queue by
-    // departure step, stable -- i.e. by (edge, departure step, id) -- queues in parallel
     const uint32_t* re = rt->route_edges;
-    std::vector<uint32_t> q_begin((size_t)E + 1, 0);
-    for (uint32_t i = 0; i < V; i++) q_begin[first_edge[i] + 1]++;
-    for (uint32_t e = 0; e < E; e++) q_begin[e + 1] += q_begin[e];
-    {
-        std::vector<uint32_t> fill(q_begin.begin(), q_begin.end() - 1);
-        for (uint32_t i = 0; i < V; i++) order[fill[first_edge[i]]++] = i;
-    }
-    parallel_chunks(E, [&](size_t b, size_t e_, size_t) {
-        for (size_t e = b; e < e_; e++)
-            if (q_begin[e + 1] - q_begin[e] > 1)
-                std::stable_sort(order.begin() + q_begin[e], order.begin() + q_begin[e + 1],
-                                 [&](uint32_t x, uint32_t y) { return dep_step[x] < dep_step[y]; });
-    });
-    // one 32-byte departure record per vehicle in queue order, one 16-byte record per queue
-    std::vector<uint4> dep_rec(2 * (size_t)V), queue_rec;
     auto fbits = [](float f) { uint32_t u; memcpy(&u, &f, 4); return u; };
-    for (uint32_t n = 0; n < V; n++) {
-        const uint32_t i = order[n], rb = route_begin[i], rend = (uint32_t)rt->route_off[i + 1];
-        const uint32_t e = re[rb];
-        if (n == 0 || e != queue_rec.back().w) {
-            if (!queue_rec.empty()) queue_rec.back().z = n;
-            queue_rec.push_back(make_uint4(edges[e].row, edges[e].lane_base, V, e));
-        }
-        const float v0m = dep->v0_mult ? dep->v0_mult[i] : 1.0f;
-        const float md = dep->mand_dist_m ? dep->mand_dist_m[i] : p->mand_dist_default;
-        dep_rec[2 * (size_t)n] = make_uint4(i, fbits(v0m), fbits(md), rb);
-        dep_rec[2 * (size_t)n + 1] = make_uint4(rend, rb + 1 < rend ? re[rb + 1] : NONE32, dep_step[i],
-                                                dep->veh_type ? dep->veh_type[i] : 0u);
+    std::vector<uint32_t> second(V), route_end(V), v0m_bits(V), mand_bits(V), type_v(V);
+    for (uint32_t i = 0; i < V; i++) {
+        const uint32_t rb = route_begin[i], rend = (uint32_t)rt->route_off[i + 1];
+        route_end[i] = rend;
+        second[i] = rb + 1 < rend ? re[rb + 1] : NONE32;
+        v0m_bits[i] = fbits(dep->v0_mult ? dep->v0_mult[i] : 1.0f);
+        mand_bits[i] = fbits(dep->mand_dist_m ? dep->mand_dist_m[i] : p->mand_dist_default);
+        type_v[i] = dep->veh_type ? dep->veh_type[i] : 0u;
     }
+    std::vector<uint4> dep_rec, queue_rec;
+    build_queues(V, E, edges, first_edge.data(), second.data(), route_begin.data(), route_end.data(), dep_step.data(),
+                 v0m_bits.data(), mand_bits.data(), type_v.data(), dep_rec, queue_rec);
     if (queue_rec.size() != L.Q) return fail(TS_EINVAL, "internal: queue count mismatch");
 
     ts_sim* s = new ts_sim();
@@ -770,6 +828,42 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         }
         chk(up(L.edge_aux, aux.data(), (size_t)E * 4));
         chk(up(L.edge_from, net->edge_from, (size_t)E * 4));
+    }
+    std::vector<uint32_t> rr_out_off, rr_out_edge, rr_origin, rr_dest, rr_src;
+    if (L.Rcap) {
+        // re-routing: the graph as CSR by tail node (edge ids ascending inside a node), every vehicle's
+        // origin and destination NODE (they never change, R38) and the list of distinct origins
+        rr_out_off.assign((size_t)N + 1, 0); rr_out_edge.resize(E);
+        for (uint32_t e = 0; e < E; e++) rr_out_off[net->edge_from[e] + 1]++;
+        for (uint32_t h = 0; h < N; h++) rr_out_off[h + 1] += rr_out_off[h];
+        { std::vector<uint32_t> fill(rr_out_off.begin(), rr_out_off.end() - 1);
+          for (uint32_t e = 0; e < E; e++) rr_out_edge[fill[net->edge_from[e]]++] = e; }
+        rr_origin.resize(V); rr_dest.resize(V); s->src_idx_h.resize(V);
+        std::vector<uint32_t> idx_of(N, NONE32);
+        for (uint32_t i = 0; i < V; i++) {
+            const uint32_t o = net->edge_from[first_edge[i]];
+            rr_origin[i] = o; rr_dest[i] = net->edge_to[re[route_end[i] - 1]];
+            if (idx_of[o] == NONE32) { idx_of[o] = (uint32_t)rr_src.size(); rr_src.push_back(o); }
+            s->src_idx_h[i] = idx_of[o];
+        }
+        chk(up(L.rr_out_off, rr_out_off.data(), ((size_t)N + 1) * 4)); chk(up(L.rr_out_edge, rr_out_edge.data(), (size_t)E * 4));
+        chk(up(L.rr_efrom, net->edge_from, (size_t)E * 4)); chk(up(L.rr_eto, net->edge_to, (size_t)E * 4));
+        chk(up(L.rr_origin, rr_origin.data(), (size_t)V * 4)); chk(up(L.rr_dest, rr_dest.data(), (size_t)V * 4));
+        chk(up(L.rr_srcidx, s->src_idx_h.data(), (size_t)V * 4)); chk(up(L.rr_src, rr_src.data(), rr_src.size() * 4));
+        chk(up(L.rr_end, route_end.data(), (size_t)V * 4));
+        s->edges_h = edges; s->dep_step_h = dep_step; s->v0m_bits_h = v0m_bits; s->mand_bits_h = mand_bits; s->type_h = type_v;
+        RrCtx& r = s->rr;
+        r.V = V; r.E = E; r.N = N; r.n_src = L.n_src;
+        r.out_off = at<uint32_t>(s, L.rr_out_off); r.out_edge = at<uint32_t>(s, L.rr_out_edge);
+        r.edge_from = at<uint32_t>(s, L.rr_efrom); r.edge_to = at<uint32_t>(s, L.rr_eto);
+        r.w = at<uint32_t>(s, L.rr_w); r.w_free = at<uint32_t>(s, L.rr_wfree);
+        r.st_exited = s->ctx.st_exited; r.st_exit_steps = s->ctx.st_exit_steps;
+        r.origin = at<uint32_t>(s, L.rr_origin); r.dest = at<uint32_t>(s, L.rr_dest); r.src_idx = at<uint32_t>(s, L.rr_srcidx);
+        r.src_node = at<uint32_t>(s, L.rr_src); r.mask = at<uint8_t>(s, L.rr_mask);
+        r.new_len = at<uint32_t>(s, L.rr_newlen); r.new_off = at<uint32_t>(s, L.rr_newoff); r.block_sum = at<uint32_t>(s, L.rr_bsum);
+        r.first2 = at<uint32_t>(s, L.rr_first2); r.pred = at<uint32_t>(s, L.rr_pred);
+        r.lab = at<unsigned long long>(s, L.rr_lab); r.fa = at<uint32_t>(s, L.rr_fa); r.fb = at<uint32_t>(s, L.rr_fb);
+        r.stamp = at<uint32_t>(s, L.rr_stamp); r.error = at<uint32_t>(s, L.rr_err);
     }
     // the staging vectors die with this scope: make sure the copies have left them
     chk(cudaStreamSynchronize(st));
@@ -1060,6 +1154,118 @@ extern "C" int ts_read_edge_stats(ts_sim* s, ts_edge_stats_out* o, int reset) {
     if (reset) {
         CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.emis - L.st_entered, s->stream));
         CUDA_TRY(cudaMemsetAsync(s->ws + L.dyn + offsetof(Dyn, n_samples), 0, 4, s->stream));
+    }
+    return TS_OK;
+}
+
+// ------------------------------------------------------------------ re-routing
+
+extern "C" int ts_reroute(ts_sim* s, const uint32_t* w_free, const uint8_t* mask, ts_reroute_out* out) {
+    if (!s || !w_free) return fail(TS_EINVAL, "null argument");
+    Layout& L = s->L;
+    if (!L.Rcap) return fail(TS_EINVAL, "the simulation was created with ts_params.route_capacity == 0");
+    if (s->sticky) return fail(TS_EINVARIANT, "sticky device error 0x%x", s->sticky);
+    const uint32_t V = L.V, E = L.E;
+    cudaStream_t st = s->stream;
+    RrCtx& r = s->rr;
+    // route tables: the one in use and the one to fill
+    uint32_t* tab[2] = {at<uint32_t>(s, L.route_edges), at<uint32_t>(s, L.rr_routes2)};
+    r.old_routes = tab[s->route_cur]; r.new_routes = tab[s->route_cur ^ 1];
+    r.old_begin = at<uint32_t>(s, L.route_begin); r.old_end = at<uint32_t>(s, L.rr_end);
+    for (uint32_t e = 0; e < E; e++)
+        if (w_free[e] < 1 || w_free[e] > kRrWMax) return fail(TS_EINVAL, "w_free[%u] = %u not in 1..2^20", e, w_free[e]);
+    CUDA_TRY(cudaMemcpyAsync(s->ws + L.rr_wfree, w_free, (size_t)E * 4, cudaMemcpyHostToDevice, st));
+    if (mask) CUDA_TRY(cudaMemcpyAsync(s->ws + L.rr_mask, mask, V, cudaMemcpyHostToDevice, st));
+    else CUDA_TRY(cudaMemsetAsync(s->ws + L.rr_mask, 1, V, st));
+    CUDA_TRY(cudaMemsetAsync(r.error, 0, 4, st));
+    // the trees wanted: origins of the vehicles asked to re-route (R39)
+    std::vector<uint8_t> want(L.n_src, 0);
+    std::vector<uint32_t> todo;
+    uint32_t n_masked = 0;
+    for (uint32_t i = 0; i < V; i++)
+        if (!mask || mask[i]) { n_masked++; if (!want[s->src_idx_h[i]]) { want[s->src_idx_h[i]] = 1; todo.push_back(s->src_idx_h[i]); } }
+    std::sort(todo.begin(), todo.end());
+    CUDA_TRY(cudaMemcpyAsync(s->ws + L.rr_todo, todo.data(), todo.size() * 4, cudaMemcpyHostToDevice, st));
+    cudaEvent_t ev[3];
+    for (auto& e : ev) CUDA_TRY(cudaEventCreate(&e));
+    k_rr_weights<<<std::max(1u, std::min(1184u, (E + 255) / 256)), 256, 0, st>>>(r);
+    CUDA_TRY(cudaEventRecord(ev[0], st));
+    if (!todo.empty())
+        k_rr_sssp<<<std::min<uint32_t>(kRrCtas, (uint32_t)todo.size()), 1024, 0, st>>>(r, at<uint32_t>(s, L.rr_todo), (uint32_t)todo.size());
+    CUDA_TRY(cudaEventRecord(ev[1], st));
+    const uint32_t vb = std::max(1u, std::min(1184u, (V + 255) / 256));
+    k_rr_len<<<vb, 256, 0, st>>>(r);
+    CUDA_TRY(cudaMemsetAsync(r.new_len + V, 0, 4, st));
+    const uint32_t n_scan = V + 1, per = kScanBlock * kScanItems, nb = (n_scan + per - 1) / per;
+    k_rr_scan1<<<nb, kScanBlock, 0, st>>>(r.new_len, r.new_off, r.block_sum, n_scan);
+    k_rr_scan2<<<1, 32, 0, st>>>(r.block_sum, nb);
+    k_rr_scan3<<<nb, kScanBlock, 0, st>>>(r.new_off, r.block_sum, n_scan);
+    CUDA_TRY(cudaGetLastError());
+    // the total decides whether the new routes fit (lengths sum below 2^32: every route has at most N edges
+    // and the scan is checked against the capacity before anything is written)
+    uint32_t total = 0, err = 0;
+    std::vector<uint32_t> new_len(V), new_off((size_t)V + 1);
+    CUDA_TRY(cudaMemcpyAsync(new_len.data(), r.new_len, (size_t)V * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(new_off.data(), r.new_off, ((size_t)V + 1) * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(&err, r.error, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (err) return fail(TS_EINVAL, "re-routing: a path cost passed 2^32 weight units");
+    uint64_t sum = 0;
+    for (uint32_t i = 0; i < V; i++) sum += new_len[i];
+    total = new_off[V];
+    if (sum > L.Rcap || sum != total) return fail(TS_ENOMEM, "re-routing: the new routes need %llu entries, route_capacity is %llu", (unsigned long long)sum, (unsigned long long)L.Rcap);
+    k_rr_write<<<vb, 256, 0, st>>>(r);
+    k_rr_first2<<<vb, 256, 0, st>>>(r);
+    CUDA_TRY(cudaEventRecord(ev[2], st));
+    CUDA_TRY(cudaGetLastError());
+    // the departure-queue index follows the new first edges (host: a counting sort and one record per vehicle)
+    std::vector<uint32_t> first2(2 * (size_t)V), first(V), second(V), rend(V);
+    CUDA_TRY(cudaMemcpyAsync(first2.data(), r.first2, (size_t)V * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (uint32_t i = 0; i < V; i++) { first[i] = first2[2 * (size_t)i]; second[i] = first2[2 * (size_t)i + 1]; rend[i] = new_off[i] + new_len[i]; }
+    std::vector<uint4> dep_rec, queue_rec;
+    build_queues(V, E, s->edges_h, first.data(), second.data(), new_off.data(), rend.data(), s->dep_step_h.data(),
+                 s->v0m_bits_h.data(), s->mand_bits_h.data(), s->type_h.data(), dep_rec, queue_rec);
+    if (queue_rec.size() > std::max(L.Q, L.Qcap)) return fail(TS_ENOMEM, "re-routing: %zu departure queues, room for %u", queue_rec.size(), std::max(L.Q, L.Qcap));
+    CUDA_TRY(cudaMemcpyAsync(s->ws + L.queue_rec, queue_rec.data(), queue_rec.size() * 16, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(s->ws + L.dep_rec, dep_rec.data(), (size_t)V * 32, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(s->ws + L.route_begin, r.new_off, (size_t)V * 4, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(s->ws + L.rr_end, rend.data(), (size_t)V * 4, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    s->route_cur ^= 1;
+    s->ctx.route_edges = tab[s->route_cur];
+    s->ctx.n_queues = (uint32_t)queue_rec.size();
+    if (out) {
+        float ms_sssp = 0, ms_all = 0;
+        cudaEventElapsedTime(&ms_sssp, ev[0], ev[1]);
+        cudaEventElapsedTime(&ms_all, ev[0], ev[2]);
+        out->n_rerouted = n_masked; out->n_trees = (uint32_t)todo.size(); out->route_entries = sum;
+        out->sssp_ms = ms_sssp; out->device_ms = ms_all;
+        if (out->w) CUDA_TRY(cudaMemcpyAsync(out->w, r.w, (size_t)E * 4, s->out_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    }
+    for (auto& e : ev) cudaEventDestroy(e);
+    return ts_reset(s);       // new demand: back to step 0, statistics cleared
+}
+
+extern "C" int ts_read_routes(ts_sim* s, uint64_t* route_off, uint32_t* route_edges, uint64_t* n_entries) {
+    if (!s) return fail(TS_EINVAL, "null sim");
+    Layout& L = s->L;
+    const uint32_t V = L.V;
+    cudaStream_t st = s->stream;
+    std::vector<uint32_t> b(V), e(V);
+    CUDA_TRY(cudaMemcpyAsync(b.data(), s->ws + L.route_begin, (size_t)V * 4, cudaMemcpyDeviceToHost, st));
+    if (L.Rcap) CUDA_TRY(cudaMemcpyAsync(e.data(), s->ws + L.rr_end, (size_t)V * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    const uint64_t total = L.Rcap ? (V ? e[V - 1] : 0) : L.R;      // routes are stored back to back in id order
+    if (n_entries) *n_entries = total;
+    if (route_off) {
+        if (s->out_on_device) return fail(TS_EINVAL, "ts_read_routes fills host arrays");
+        for (uint32_t i = 0; i < V; i++) route_off[i] = b[i];
+        route_off[V] = total;
+    }
+    if (route_edges) {
+        CUDA_TRY(cudaMemcpyAsync(route_edges, s->ctx.route_edges, total * 4, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
     }
     return TS_OK;
 }

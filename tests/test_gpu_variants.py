@@ -79,14 +79,15 @@ def test_validation_of_the_new_inputs(cfg1):
         dict(cfg1, params=dict(cfg1["params"], n_types=2, type_len=(5, 1, 0, 0), type_a=(1, 1, 0, 0), type_vmax=(9, 9, 0, 0))),
         dict(cfg1, veh_type=np.full(cfg1["n_vehicles"], 1, np.uint8)),                       # type 1 without types
         dict(cfg1, node_ctrl=np.full(cfg1["n_nodes"], 5, np.uint8)),
-        dict(cfg1, params=dict(cfg1["params"], lookahead_cells=16)),                         # shorter than a step + a vehicle
+        corridor(vlim=29.0, params=dict(lookahead_cells=16)),                                # shorter than a step + a vehicle
         dict(cfg1, params=dict(cfg1["params"], lookback_cells=0)),
         dict(W.with_controls(cfg1), params=dict(W.with_controls(cfg1)["params"], n_types=1, type_len=(15.5, 0, 0, 0),
                                                 type_a=(1, 0, 0, 0), type_vmax=(99, 0, 0, 0), entry_zone_cells=40)),
     ]
-    for b in bad:
+    for n, b in enumerate(bad):
         with pytest.raises(pkg.TsError) as e:
             pkg.Sim(b, "cuda:0")
+            pytest.fail(f"case {n} was accepted")
         assert e.value.code == pkg.binding.TS_EINVAL
 
 
