@@ -209,6 +209,86 @@ def run_reference(args):
     }))
 
 
+def run_reroute(args):
+    """--reroute: the paper's assignment loop: simulate, measure, re-route all / all /
+    half / a quarter of the vehicles, four times; one bench "step" is the whole loop.  Prints the
+    usual line (vehicle-updates/s over the loop, ts_reroute included) plus a `reroute` object with
+    the per-iteration gap between the times the routes were chosen with and the times simulated,
+    and a roofline object for the shortest-path kernel."""
+    import torch
+    import paper_1807_01148_b200 as pkg
+    from paper_1807_01148_b200 import workload as W
+    torch.cuda.set_device(0)
+    bundle = load_workload(args.workload)
+    cap = int(len(bundle["route_edges"]) * 2 + 1024)
+    b = dict(bundle, params=dict(bundle["params"], route_capacity=cap))
+    sim = pkg.Sim(b, "cuda:0")
+    stream = torch.cuda.current_stream()
+    wf = W.free_flow_weights(b)
+    steps = args.sim_steps or b["steps"]
+    E, dt = b["n_edges"], b["params"]["dt"]
+    rows, ms_all, updates_all, launches = [], [], [], 0
+    sampler = ClockSampler(0)
+    for rep_ in range(args.warmup + args.steps):
+        if rep_ == args.warmup:
+            sampler.start()
+        if rep_:                                        # every repetition starts from the routes given
+            sim.close()
+            sim = pkg.Sim(b, "cuda:0")
+        used = wf.astype(np.float64) / W.W_UNIT          # weights the routes in use were chosen with, in steps
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        upd, rows = 0, []
+        for it in range(4):
+            sim.step(steps)
+            st = sim.read_counts()
+            upd += int(st["vehicle_updates"])
+            es = sim.read_edge_stats()
+            seen = es["exited"] > 0
+            sim_t = es["exit_steps_sum"][seen] / es["exited"][seen]
+            t_host = time.perf_counter()
+            info = sim.reroute(wf, W.reroute_mask(b["n_vehicles"], it))
+            host_ms = 1e3 * (time.perf_counter() - t_host)
+            rows.append({"iteration": it, "n_rerouted": info["n_rerouted"], "n_trees": info["n_trees"],
+                         "sssp_ms": info["sssp_ms"], "device_ms": info["device_ms"], "call_ms": host_ms,
+                         "arrived": int(st["n_arrived"]), "edges_with_exits": int(seen.sum()),
+                         "mean_abs_gap_s": float(np.abs(used[seen] - sim_t).mean() * dt),
+                         "mean_simulated_s": float(sim_t.mean() * dt)})
+            used = info["w"].astype(np.float64) / W.W_UNIT
+        e1.record(stream)
+        torch.cuda.synchronize()
+        if rep_ >= args.warmup:
+            ms_all.append(e0.elapsed_time(e1)); updates_all.append(upd)
+            launches += 4 * (2 * ((steps + 2047) // 2048) + 9)
+    clocks = sampler.stop()
+    sim.close()
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    peak = float(json.load(open(peaks_path))["hbm_gbs"]) if os.path.exists(peaks_path) else 6650.0
+    trees = sum(r["n_trees"] for r in rows)
+    sssp_s = sum(r["sssp_ms"] for r in rows) / 1e3
+    # per tree every edge is relaxed at least once: label of the tail (8 B), out_edge + edge_to + weight
+    # (12 B), label of the head read and written by the atomicMin (16 B)
+    alg = 36.0 * E * trees
+    value = sum(updates_all) / (sum(ms_all) / 1e3)
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": sum(ms_all) / len(ms_all), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 (traffic), u32/u64 (routing weights and labels)", "data": "synthetic",
+        "config": {"workload": bundle["name"] + " + 4 re-routing iterations (PAPER.md:386)", "vehicles": b["n_vehicles"],
+                   "edges": E, "sim_steps_per_iteration": steps},
+        "reroute": rows, "gpu_launches": launches, "clocks": clocks,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": int(4 * (E * 4 + b["n_vehicles"])),
+                "d2h_bytes_per_step": int(4 * (E * 28 + b["n_vehicles"] * 16)),
+                "note": "the loop is driven through the C ABI: statistics D2H, masks and free-flow weights H2D, "
+                        "the departure-queue index rebuilt on the host inside ts_reroute"},
+        "roofline": {"bound": "hbm", "kernel": "k_rr_sssp", "achieved": alg / sssp_s / 1e9 if sssp_s else None, "peak": peak,
+                     "unit": "GB/s", "frac": alg / sssp_s / 1e9 / peak if sssp_s else None, "traffic": None,
+                     "bytes_per_unit": 36.0, "unit_of_work": "edge relaxation (one per edge per tree at least)",
+                     "trees": trees, "kernel_ms_total": 1e3 * sssp_s},
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -229,9 +309,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end leg (profiling runs)")
     ap.add_argument("--no-window", action="store_true", help="skip the busiest-window pass (profiling runs)")
+    ap.add_argument("--reroute", action="store_true",
+                    help="the four-iteration re-routing loop of PAPER.md:386 on the workload (SURVEY.md 8(f) row 1)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.reroute:
+        return run_reroute(args)
     if args.warmup < 3:
         print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
 

@@ -501,6 +501,27 @@ def reroute_mask(n_vehicles, iteration, seed=0):
     return (rng.random(n_vehicles) < share).astype(np.uint8)
 
 
+# --------------------------------------------------------------------------- static assignment inputs
+
+def sue_inputs(bundle, horizon_s=3600.0):
+    """Inputs of the static user equilibrium of PAPER.md:307-338 for a config's network and demand:
+    free-flow time t0 = length / speed (Eq. 4), capacity per edge in vehicles per second
+    from a per-lane hourly capacity by road class (Table 2 gives 800-2200 per lane per
+    hour by OpenStreetMap type, which synthetic edges do not have: 2200 for >= 4 lanes, 1000 for a
+    limit >= 17 m/s, else 900), and the OD matrix as integer trips per (origin node, destination
+    node) pair, the demand rate being trips per `horizon_s`."""
+    b = bundle
+    t0 = b["edge_len_m"].astype(np.float64) / b["edge_vlim"].astype(np.float64)
+    per_lane = np.where(b["edge_lanes"] >= 4, 2200.0, np.where(b["edge_vlim"] >= 17.0, 1000.0, 900.0))
+    cap = per_lane * b["edge_lanes"].astype(np.float64) / 3600.0
+    off = b["route_off"].astype(np.int64)
+    o = b["edge_from"][b["route_edges"][off[:-1]]].astype(np.int64)
+    d = b["edge_to"][b["route_edges"][off[1:] - 1]].astype(np.int64)
+    key, trips = np.unique(o * b["n_nodes"] + d, return_counts=True)
+    return dict(t0=t0, cap=cap * horizon_s, od_origin=(key // b["n_nodes"]).astype(np.uint32),
+                od_dest=(key % b["n_nodes"]).astype(np.uint32), od_trips=trips.astype(np.uint32))
+
+
 _BY_NAME = {
     "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5,
     "cfg3_dense": config3_dense,
