@@ -241,6 +241,39 @@ int ts_reroute(ts_sim *sim, const uint32_t *w_free, const uint8_t *mask, ts_rero
  * call once with both NULL to learn *n_entries).  Synchronises. */
 int ts_read_routes(ts_sim *sim, uint64_t *route_off, uint32_t *route_edges, uint64_t *n_entries);
 
+/* Static user equilibrium by the Frank-Wolfe algorithm with BPR travel times -- the paper's static
+ * traffic assignment model, PAPER.md:307-338 (section 5.3: steps 1-4, objective Eq. 6) with the BPR
+ * curve of PAPER.md:200-216 (Eq. 3: t = t0 (1 + alpha (v/c)^beta), beta = 4).  A self-contained call
+ * on the same shortest-path kernel as ts_reroute.  Readings R42-R44 of DESIGN.md: beta is the integer
+ * 4; the all-or-nothing step grows its trees on integer weights max(1, rint(t * weight_scale)) with
+ * the tie-break of ts_reroute; demand is integer trips per OD pair.
+ * All arrays of ts_sue_problem are HOST arrays; flow / time of ts_sue_out are HOST arrays [E] unless
+ * ts_device.out_on_device; objective [iterations + 1], gap and step [iterations] are always host (any
+ * may be NULL).  gap[k] = (x.t - y.t) / x.t before step k (0 at equilibrium, Wardrop's condition,
+ * PAPER.md:313); step[k] in [0, 1] by bisection on the derivative along the segment; objective[k] =
+ * Eq. 6 at x_k.  fp64.  Synchronises.  Errors: TS_EINVAL, TS_ENOMEM (workspace), TS_ECUDA. */
+typedef struct ts_sue_problem {
+    uint32_t n_nodes, n_edges;
+    const uint32_t *edge_from, *edge_to;   /* [E] */
+    const double *t0;                      /* [E] free-flow time (Eq. 4), > 0 */
+    const double *cap;                     /* [E] capacity in the demand's unit of time, > 0 */
+    uint32_t n_od;
+    const uint32_t *od_origin, *od_dest;   /* [n_od] nodes */
+    const uint32_t *od_trips;              /* [n_od] */
+    double alpha;                          /* 0.15 */
+    double weight_scale;                   /* integer weight = max(1, rint(t * weight_scale)), <= 2^20 */
+    uint32_t iterations;                   /* Frank-Wolfe iterations after the initial assignment */
+    uint32_t bisections;                   /* of the line search, <= 64 */
+} ts_sue_problem;
+typedef struct ts_sue_out {
+    double *flow, *time;
+    double *objective, *gap, *step;
+    float device_ms, sssp_ms;              /* device time of the whole solve / of the tree kernel */
+    uint32_t n_trees;
+} ts_sue_out;
+int ts_sue_workspace(const ts_sue_problem *problem, size_t *bytes);
+int ts_sue_solve(const ts_sue_problem *problem, const ts_device *dev, ts_sue_out *out);
+
 /* Tuning knobs that never change results.
  *  "mode"          1 (default) = ts_step(n) is ONE persistent cooperative kernel looping over
  *                  the n steps with grid-wide barriers; 0 = one launch per phase.

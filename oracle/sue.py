@@ -15,7 +15,7 @@ beta = 4).  Plain numpy in fp64, step by step in the paper's order:
 with f(x) = sum_e integral_0^{x_e} t_e(s) ds = sum_e t0_e (x_e + alpha x_e^5 / (5 c_e^4))  (Eq. 6).
 
 Readings (R42-R44): beta is the integer 4 (two squarings); the all-or-nothing step uses
-shortest paths on INTEGER weights w_e = max(1, rint(t_e * weight_scale)) with the tie-break of the
+shortest paths on INTEGER weights w_e = rint(t_e * weight_scale) clamped to [1, 2^20] with the tie-break of the
 re-routing oracle (oracle/reroute.py, R38), so that the discrete part of the iteration does not hang
 on floating-point ties; demand is integer trips per OD pair.
 Only tests/ and bench.py's oracle legs may import this module; it imports nothing from the package.
@@ -44,7 +44,7 @@ def objective(t0, cap, x, alpha=ALPHA):
 
 
 def weights(t, weight_scale):
-    return np.maximum(1, np.rint(t * weight_scale)).astype(np.uint32)
+    return np.clip(np.rint(t * weight_scale), 1, 1 << 20).astype(np.uint32)
 
 
 def all_or_nothing(n_nodes, edge_from, edge_to, w, od_origin, od_dest, od_trips):

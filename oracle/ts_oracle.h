@@ -1,10 +1,11 @@
 /*
  * ts_oracle.h -- ORACLE (test infrastructure, not product code).
  *
- * A plain, slow, single-threaded CPU restatement of the per-vehicle traffic
+ * A plain, slow CPU restatement (single-threaded unless orc_set_threads is called) of the per-vehicle traffic
  * microsimulation of arxiv 1807.01148 (sections 6.3.2-6.3.3), following
- * SURVEY.md section 8(c) step by step (readings R1-R27 are listed in DESIGN.md; R27 fixes the
- * rounding order of two quotients inside Eq. 7).
+ * SURVEY.md section 8(c) step by step (readings R1-R36 are listed in DESIGN.md; R27 fixes the
+ * rounding order of two quotients inside Eq. 7; R31 vehicle types; R34-R36 the control
+ * variants of PAPER.md:402).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
  * may load this library.  It shares no code, header, table or helper with the CUDA path
@@ -25,15 +26,21 @@
  * queue's idle totals, a cruising vehicle, and a fine-step fp64 quadrature of the lone-vehicle
  * acceleration run).
  *
- * Parity pins (tests/test_oracle_pins.py, test_oracle_invariants.py, test_oracle_scenarios.py):
- * P1 lone-vehicle closed form, P2 platoon equilibrium gap, P3 standing queue, I1-I8 invariants,
- * P4 brute force, P5 degenerate cases; scenario pins re-derived in fp64 from the rule text: the
- * discretionary lane-change decision with an empty target lane (incentive vs threshold on every
- * turn), gap acceptance at the moment of every change, hold-at-line after a lost claim with the
- * lowest id first, departure order and entry clearance.
- * PARITY UNPINNED against the outside world (pinned oracle<->GPU only): the VALUE of the MOBIL
- * politeness term (new follower's loss) and of the mandatory-change threshold; these have no
- * statement in the paper beyond PAPER.md:399-400 to pin them to.
+ * Parity pins (tests/test_oracle_pins.py, test_oracle_invariants.py, test_oracle_scenarios.py,
+ * test_oracle_lane_change_referee.py, test_oracle_variants.py):
+ * P1 lone-vehicle closed form, P2 platoon equilibrium gap (on one edge, across nodes, behind a truck),
+ * P3 standing queue, I1-I8 invariants, P4 brute force, P5 degenerate cases; a referee that re-derives
+ * in fp64, from the rule text, EVERY lane-change decision of dense multi-lane scenarios (eligibility,
+ * G1, G2 with its kinematic bound, G3, the mandatory rule at the first eligible turn, the veto of a
+ * discretionary move into a lane that ends, the MOBIL incentive with the politeness term deciding both
+ * ways) and is shown to catch the mutations a reviewer would try (dropped `m` term, flipped b_safe
+ * sign, dropped politeness, `>=` -> `>`, dropped `+cL2`, `cF+1` -> `cF`); hold-at-line after a lost
+ * claim; departure order and entry clearance; vehicle types (P1/P2 with the truck's own a, length and
+ * cap; bodies never overlap); STOP control, n*m phases and amber checked from the recorded states
+ * against the rule text and explicit timetables.  No sub-rule of vehicle_intent() is left pinned
+ * oracle<->GPU only; what the PAPER does not fix (the readings R1-R44) is listed in DESIGN.md.
+ * orc_set_threads: the intent loop may run on several host threads (results identical, tested);
+ * the default and bench.py's cpu_baseline are single-threaded.
  */
 #ifndef TS_ORACLE_H
 #define TS_ORACLE_H

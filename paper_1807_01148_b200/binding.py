@@ -17,7 +17,7 @@ TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
            "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile",
-           "ts_read_emissions", "ts_reroute", "ts_read_routes", "ts_destroy", "ts_last_error", "ts_version"]
+           "ts_read_emissions", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_destroy", "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -77,6 +77,18 @@ class TsRerouteOut(C.Structure):
                 ("sssp_ms", C.c_float), ("device_ms", C.c_float), ("w", C.c_void_p)]
 
 
+class TsSueProblem(C.Structure):
+    _fields_ = [("n_nodes", C.c_uint32), ("n_edges", C.c_uint32), ("edge_from", C.c_void_p), ("edge_to", C.c_void_p),
+                ("t0", C.c_void_p), ("cap", C.c_void_p), ("n_od", C.c_uint32), ("od_origin", C.c_void_p),
+                ("od_dest", C.c_void_p), ("od_trips", C.c_void_p), ("alpha", C.c_double), ("weight_scale", C.c_double),
+                ("iterations", C.c_uint32), ("bisections", C.c_uint32)]
+
+
+class TsSueOut(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("flow", "time", "objective", "gap", "step")] + \
+               [("device_ms", C.c_float), ("sssp_ms", C.c_float), ("n_trees", C.c_uint32)]
+
+
 class TsError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__(f"ts error {code}: {msg}")
@@ -110,7 +122,9 @@ def load():
         L.ts_destroy.restype = None
         L.ts_last_error.restype = C.c_char_p
         L.ts_version.restype = C.c_char_p
-        for n in EXPORTS[:12]:
+        L.ts_sue_workspace.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ts_sue_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        for n in EXPORTS[:14]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -280,3 +294,31 @@ def utilisation(edge_stats, bundle):
     cap = bundle["edge_len_m"].astype(np.float64) * bundle["edge_lanes"] / (p["veh_len"] + p["s0"])
     n = max(1, int(edge_stats["n_samples"]))
     return edge_stats["sample_count_sum"] / n / cap
+
+
+def sue_solve(n_nodes, edge_from, edge_to, t0, cap, od_origin, od_dest, od_trips, iterations=20, bisections=40,
+              weight_scale=1000.0, alpha=0.15, device="cuda:0"):
+    """ts_sue_solve: static user equilibrium by Frank-Wolfe with BPR times.
+    Marshalling only; returns (flow, time, dict(objective, gap, step, device_ms, sssp_ms, n_trees))."""
+    import torch
+    L = load()
+    u32 = lambda a: np.ascontiguousarray(a, np.uint32)
+    f64 = lambda a: np.ascontiguousarray(a, np.float64)
+    keep = [u32(edge_from), u32(edge_to), f64(t0), f64(cap), u32(od_origin), u32(od_dest), u32(od_trips)]
+    E, n_od = len(keep[0]), len(keep[4])
+    prob = TsSueProblem(int(n_nodes), E, keep[0].ctypes.data, keep[1].ctypes.data, keep[2].ctypes.data,
+                        keep[3].ctypes.data, n_od, keep[4].ctypes.data, keep[5].ctypes.data, keep[6].ctypes.data,
+                        float(alpha), float(weight_scale), int(iterations), int(bisections))
+    n = C.c_size_t()
+    _check(L.ts_sue_workspace(C.byref(prob), C.byref(n)))
+    dev_t = torch.device(device)
+    torch.cuda.set_device(dev_t)
+    ws = torch.empty(n.value + 256, dtype=torch.uint8, device=dev_t)
+    base = (ws.data_ptr() + 255) & ~255
+    dev = TsDevice(base, n.value, torch.cuda.current_stream(dev_t).cuda_stream, 0)
+    flow, time_ = np.zeros(E), np.zeros(E)
+    obj, gap, step = np.zeros(iterations + 1), np.zeros(iterations), np.zeros(iterations)
+    out = TsSueOut(flow.ctypes.data, time_.ctypes.data, obj.ctypes.data, gap.ctypes.data, step.ctypes.data)
+    _check(L.ts_sue_solve(C.byref(prob), C.byref(dev), C.byref(out)))
+    return flow, time_, dict(objective=obj, gap=gap, step=step, device_ms=out.device_ms, sssp_ms=out.sssp_ms,
+                             n_trees=out.n_trees, workspace_bytes=n.value)

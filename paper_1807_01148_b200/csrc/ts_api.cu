@@ -23,6 +23,7 @@
 #include "ts_phases.cuh"
 #include "ts_sort.cuh"
 #include "ts_reroute.cuh"
+#include "ts_sue.cuh"
 
 namespace cg = cooperative_groups;
 using namespace ts;
@@ -1267,5 +1268,167 @@ extern "C" int ts_read_routes(ts_sim* s, uint64_t* route_off, uint32_t* route_ed
         CUDA_TRY(cudaMemcpyAsync(route_edges, s->ctx.route_edges, total * 4, cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaStreamSynchronize(st));
     }
+    return TS_OK;
+}
+
+// ------------------------------------------------------------------ static user equilibrium
+
+struct SueLayout {
+    size_t total = 0;
+    size_t out_off, out_edge, efrom, eto, t0, cap, x, t, w, y, part, od_o, od_d, od_t, od_s, src, todo, pred, lab, fa, fb, stamp, err;
+    uint32_t n_src = 0;
+    size_t take(size_t bytes) { size_t off = total; total += (bytes + 255) & ~(size_t)255; return off; }
+    void plan(uint32_t N, uint32_t E, uint32_t n_od) {
+        out_off = take(((size_t)N + 1) * 4); out_edge = take((size_t)E * 4); efrom = take((size_t)E * 4); eto = take((size_t)E * 4);
+        t0 = take((size_t)E * 8); cap = take((size_t)E * 8); x = take((size_t)E * 8); t = take((size_t)E * 8);
+        w = take((size_t)E * 4); y = take((size_t)E * 8); part = take((size_t)kSueBlocks * 2 * 8);
+        od_o = take((size_t)n_od * 4); od_d = take((size_t)n_od * 4); od_t = take((size_t)n_od * 4); od_s = take((size_t)n_od * 4);
+        src = take((size_t)n_src * 4); todo = take((size_t)n_src * 4); pred = take((size_t)n_src * N * 4);
+        lab = take((size_t)kRrCtas * N * 8); fa = take((size_t)kRrCtas * N * 4); fb = take((size_t)kRrCtas * N * 4);
+        stamp = take((size_t)kRrCtas * N * 4); err = take(4);
+    }
+};
+
+static int sue_plan(const ts_sue_problem* p, SueLayout& L, std::vector<uint32_t>* src_nodes, std::vector<uint32_t>* od_src) {
+    if (!p || !p->edge_from || !p->edge_to || !p->t0 || !p->cap || (p->n_od && (!p->od_origin || !p->od_dest || !p->od_trips)))
+        return fail(TS_EINVAL, "null argument");
+    if (p->n_nodes == 0 || p->n_edges == 0) return fail(TS_EINVAL, "empty network");
+    if (!(p->alpha >= 0) || !(p->weight_scale > 0) || p->bisections > 64) return fail(TS_EINVAL, "alpha >= 0, weight_scale > 0, bisections <= 64");
+    for (uint32_t e = 0; e < p->n_edges; e++) {
+        if (p->edge_from[e] >= p->n_nodes || p->edge_to[e] >= p->n_nodes) return fail(TS_EINVAL, "edge %u: endpoint out of range", e);
+        if (!(p->t0[e] > 0) || !(p->cap[e] > 0)) return fail(TS_EINVAL, "edge %u: t0 and cap must be > 0", e);
+    }
+    std::vector<uint32_t> idx_of(p->n_nodes, NONE32), srcs;
+    if (od_src) od_src->resize(p->n_od);
+    for (uint32_t q = 0; q < p->n_od; q++) {
+        if (p->od_origin[q] >= p->n_nodes || p->od_dest[q] >= p->n_nodes) return fail(TS_EINVAL, "OD pair %u: node out of range", q);
+        const uint32_t o = p->od_origin[q];
+        if (idx_of[o] == NONE32) { idx_of[o] = (uint32_t)srcs.size(); srcs.push_back(o); }
+        if (od_src) (*od_src)[q] = idx_of[o];
+    }
+    L.n_src = (uint32_t)srcs.size();
+    L.plan(p->n_nodes, p->n_edges, p->n_od);
+    if (src_nodes) *src_nodes = srcs;
+    return TS_OK;
+}
+
+extern "C" int ts_sue_workspace(const ts_sue_problem* p, size_t* bytes) {
+    if (!bytes) return fail(TS_EINVAL, "bytes is null");
+    SueLayout L;
+    int rc = sue_plan(p, L, nullptr, nullptr);
+    if (rc) return rc;
+    *bytes = L.total;
+    return TS_OK;
+}
+
+extern "C" int ts_sue_solve(const ts_sue_problem* p, const ts_device* dev, ts_sue_out* out) {
+    if (!dev || !out) return fail(TS_EINVAL, "null argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(TS_ECUDA, "no CUDA device: this library has no CPU fallback");
+    SueLayout L;
+    std::vector<uint32_t> srcs, od_src;
+    int rc = sue_plan(p, L, &srcs, &od_src);
+    if (rc) return rc;
+    if (!dev->workspace || ((uintptr_t)dev->workspace & 255)) return fail(TS_EINVAL, "workspace must be a 256-byte aligned device pointer");
+    if (dev->bytes < L.total) return fail(TS_ENOMEM, "workspace too small: %zu < %zu bytes", dev->bytes, L.total);
+    uint8_t* ws = (uint8_t*)dev->workspace;
+    cudaStream_t st = (cudaStream_t)dev->cuda_stream;
+    const uint32_t N = p->n_nodes, E = p->n_edges, n_od = p->n_od;
+    std::vector<uint32_t> out_off((size_t)N + 1, 0), out_edge(E), todo(L.n_src);
+    for (uint32_t e = 0; e < E; e++) out_off[p->edge_from[e] + 1]++;
+    for (uint32_t h = 0; h < N; h++) out_off[h + 1] += out_off[h];
+    { std::vector<uint32_t> fill(out_off.begin(), out_off.end() - 1);
+      for (uint32_t e = 0; e < E; e++) out_edge[fill[p->edge_from[e]]++] = e; }
+    for (uint32_t i = 0; i < L.n_src; i++) todo[i] = i;
+    auto up = [&](size_t off, const void* src, size_t bytes) { return bytes ? cudaMemcpyAsync(ws + off, src, bytes, cudaMemcpyHostToDevice, st) : cudaSuccess; };
+    CUDA_TRY(up(L.out_off, out_off.data(), ((size_t)N + 1) * 4)); CUDA_TRY(up(L.out_edge, out_edge.data(), (size_t)E * 4));
+    CUDA_TRY(up(L.efrom, p->edge_from, (size_t)E * 4)); CUDA_TRY(up(L.eto, p->edge_to, (size_t)E * 4));
+    CUDA_TRY(up(L.t0, p->t0, (size_t)E * 8)); CUDA_TRY(up(L.cap, p->cap, (size_t)E * 8));
+    CUDA_TRY(up(L.od_o, p->od_origin, (size_t)n_od * 4)); CUDA_TRY(up(L.od_d, p->od_dest, (size_t)n_od * 4));
+    CUDA_TRY(up(L.od_t, p->od_trips, (size_t)n_od * 4)); CUDA_TRY(up(L.od_s, od_src.data(), (size_t)n_od * 4));
+    CUDA_TRY(up(L.src, srcs.data(), (size_t)L.n_src * 4)); CUDA_TRY(up(L.todo, todo.data(), (size_t)L.n_src * 4));
+    CUDA_TRY(cudaMemsetAsync(ws + L.err, 0, 4, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    auto dp = [&](size_t off) { return reinterpret_cast<double*>(ws + off); };
+    auto up32 = [&](size_t off) { return reinterpret_cast<uint32_t*>(ws + off); };
+    RrCtx r;
+    memset(&r, 0, sizeof r);
+    r.N = N; r.E = E; r.n_src = L.n_src;
+    r.out_off = up32(L.out_off); r.out_edge = up32(L.out_edge); r.edge_from = up32(L.efrom); r.edge_to = up32(L.eto);
+    r.w = up32(L.w); r.src_node = up32(L.src); r.pred = up32(L.pred);
+    r.lab = reinterpret_cast<unsigned long long*>(ws + L.lab); r.fa = up32(L.fa); r.fb = up32(L.fb); r.stamp = up32(L.stamp);
+    r.error = up32(L.err);
+    unsigned long long* y = reinterpret_cast<unsigned long long*>(ws + L.y);
+    const uint32_t eb = std::max(1u, std::min(1184u, (E + 255) / 256)), ob = std::max(1u, std::min(1184u, (n_od + 255) / 256));
+    cudaEvent_t ev0, ev1, t0e, t1e;
+    CUDA_TRY(cudaEventCreate(&ev0)); CUDA_TRY(cudaEventCreate(&ev1)); CUDA_TRY(cudaEventCreate(&t0e)); CUDA_TRY(cudaEventCreate(&t1e));
+    float sssp_ms = 0;
+    double part[2 * kSueBlocks];
+    // one all-or-nothing assignment on the times of flow x (nullptr: free flow) into y
+    auto assign = [&](const double* x) -> int {
+        k_sue_times<<<eb, 256, 0, st>>>(E, dp(L.t0), dp(L.cap), x, p->alpha, p->weight_scale, dp(L.t), r.w);
+        CUDA_TRY(cudaEventRecord(t0e, st));
+        if (L.n_src) k_rr_sssp<<<std::min<uint32_t>(kRrCtas, L.n_src), 1024, 0, st>>>(r, up32(L.todo), L.n_src);
+        CUDA_TRY(cudaEventRecord(t1e, st));
+        CUDA_TRY(cudaMemsetAsync(y, 0, (size_t)E * 8, st));
+        if (n_od) k_sue_aon<<<ob, 256, 0, st>>>(n_od, up32(L.od_o), up32(L.od_d), up32(L.od_t), up32(L.od_s), r.pred, N, r.edge_from, y);
+        CUDA_TRY(cudaGetLastError());
+        CUDA_TRY(cudaEventSynchronize(t1e));
+        float ms = 0; cudaEventElapsedTime(&ms, t0e, t1e); sssp_ms += ms;
+        return TS_OK;
+    };
+    // block sums added up in block order on the host: the same sum whatever the scheduling
+    auto reduce = [&](int mode, double a, double& s0, double& s1) -> int {
+        k_sue_reduce<<<kSueBlocks, kSueThreads, 0, st>>>(mode, E, dp(L.t0), dp(L.cap), dp(L.x), y, a, p->alpha, dp(L.part));
+        CUDA_TRY(cudaMemcpyAsync(part, ws + L.part, sizeof part, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        s0 = s1 = 0.0;
+        for (uint32_t b = 0; b < kSueBlocks; b++) { s0 += part[b]; s1 += part[kSueBlocks + b]; }
+        return TS_OK;
+    };
+    CUDA_TRY(cudaEventRecord(ev0, st));
+    double s0, s1;
+    if ((rc = assign(nullptr))) return rc;                                     // step 1: x_0
+    k_sue_update<<<eb, 256, 0, st>>>(E, dp(L.x), y, 0.0, 1);
+    if ((rc = reduce(1, 0.0, s0, s1))) return rc;
+    if (out->objective) out->objective[0] = s0;
+    for (uint32_t k = 0; k < p->iterations; k++) {
+        if ((rc = assign(dp(L.x)))) return rc;                                 // step 2: y_k
+        if ((rc = reduce(2, 0.0, s0, s1))) return rc;
+        if (out->gap) out->gap[k] = (s0 - s1) / s0;
+        double a, g1, g0;                                                      // step 3: step length
+        if ((rc = reduce(0, 1.0, g1, s1))) return rc;
+        if (g1 <= 0.0) a = 1.0;
+        else {
+            if ((rc = reduce(0, 0.0, g0, s1))) return rc;
+            if (g0 >= 0.0) a = 0.0;
+            else {
+                double lo = 0.0, hi = 1.0;
+                for (uint32_t b = 0; b < p->bisections; b++) {
+                    const double mid = 0.5 * (lo + hi);
+                    double g;
+                    if ((rc = reduce(0, mid, g, s1))) return rc;
+                    if (g > 0.0) hi = mid; else lo = mid;
+                }
+                a = 0.5 * (lo + hi);
+            }
+        }
+        k_sue_update<<<eb, 256, 0, st>>>(E, dp(L.x), y, a, 0);                 // step 4
+        if (out->step) out->step[k] = a;
+        if ((rc = reduce(1, 0.0, s0, s1))) return rc;
+        if (out->objective) out->objective[k + 1] = s0;
+    }
+    k_sue_times<<<eb, 256, 0, st>>>(E, dp(L.t0), dp(L.cap), dp(L.x), p->alpha, p->weight_scale, dp(L.t), r.w);
+    CUDA_TRY(cudaEventRecord(ev1, st));
+    const cudaMemcpyKind kind = dev->out_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (out->flow) CUDA_TRY(cudaMemcpyAsync(out->flow, ws + L.x, (size_t)E * 8, kind, st));
+    if (out->time) CUDA_TRY(cudaMemcpyAsync(out->time, ws + L.t, (size_t)E * 8, kind, st));
+    uint32_t err = 0;
+    CUDA_TRY(cudaMemcpyAsync(&err, ws + L.err, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    float ms = 0; cudaEventElapsedTime(&ms, ev0, ev1);
+    out->device_ms = ms; out->sssp_ms = sssp_ms; out->n_trees = L.n_src * (p->iterations + 1);
+    cudaEventDestroy(ev0); cudaEventDestroy(ev1); cudaEventDestroy(t0e); cudaEventDestroy(t1e);
+    if (err) return fail(TS_EINVAL, "a path cost passed 2^32 weight units: lower weight_scale");
     return TS_OK;
 }

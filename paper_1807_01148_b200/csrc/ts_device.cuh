@@ -219,6 +219,21 @@ __device__ __forceinline__ float idm(const Params& p, float a, float Kinv, float
     float d = fr - q2;
     return a * d;
 }
+// The same in two pieces, so that the free-road factor of one (v, v0) is formed once and several
+// interactions are evaluated side by side (independent chains: the scheduler overlaps them).
+__device__ __forceinline__ float idm_follow(const Params& p, float a, float Kinv, float fr, float v, float s, float dv) {
+    float t = v * p.T;
+    float u = v * dv;
+    float w = u * Kinv;
+    t = t + w;
+    t = fmaxf(t, 0.0f);
+    float ss = p.s0 + t;
+    float se = fmaxf(s, 0.5f);
+    float q = ss / se;
+    float q2 = q * q;
+    float d = fr - q2;
+    return a * d;
+}
 
 // Section 6.3.4.  Eq. 8: grams of CO per second at speed v; the paper's v_m is
 // in miles per hour, 1 m/s = 2.2369363 mph (reading R28).

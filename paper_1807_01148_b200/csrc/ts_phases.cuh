@@ -171,6 +171,16 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     }
     const float dv_lead = v - speed_decode(code_lead);
 
+    // Eq. 7 against the own leader, the stop line and (below) the target lane: every evaluation is
+    // spelled out unconditionally and the rule picks afterwards -- the chains are independent, so they
+    // overlap instead of queueing behind one another's branches (the values are the same either way)
+    const float fr = idm_free(v, v0);
+    const float acc_free = a_i * fr;
+    const float acc_follow = idm_follow(p, a_i, Kinv_i, fr, v, s_lead, dv_lead);
+    const float acc_stop = idm_follow(p, a_i, Kinv_i, fr, v, Cf - x, v);             // 2c
+    float acc = has_lead ? acc_follow : acc_free;
+    if (!may_cross) acc = fminf(acc, acc_stop);
+
     // 2d gap acceptance G1-G3, then the mandatory rule or the MOBIL incentive G4
     bool accepted = false;
     const bool has_Lt = cLt >= 0;
@@ -184,44 +194,34 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
         const float a_F_ = EXT ? p.t_a[ty_F & 3u] : p.a, Kinv_F = EXT ? p.t_Kinv[ty_F & 3u] : p.Kinv;
         const float half_a_dt_F = EXT ? p.t_half_a_dt[ty_F & 3u] : p.half_a_dt;
         const float v0F = EXT ? fminf(E.vlim, p.t_vmax[ty_F & 3u]) : E.vlim;
-        float s_lag = 0.0f;
-        if (has_Lt) { s_Lt = (float)cLt - len_Lt; s_Lt = s_Lt - x; }
-        if (has_F) { s_lag = x - len_i; s_lag = s_lag - (float)(cF + 1); }
-        bool ok = !has_Lt || s_Lt >= p.s0;                                   // G1
-        float aF_new = 0.0f;
-        if (ok && has_F) {                                                   // G2 (E4)
-            float m = (vF + 0.125f) + half_a_dt_F;
-            m = m * p.dt;
-            ok = s_lag >= p.s0 && s_lag >= m;
+        s_Lt = (float)cLt - len_Lt; s_Lt = s_Lt - x;                         // used only where has_Lt
+        float s_lag = x - len_i; s_lag = s_lag - (float)(cF + 1);             // used only where has_F
+        float m = (vF + 0.125f) + half_a_dt_F;                               // E4
+        m = m * p.dt;
+        float sF = (float)cLt - len_Lt;
+        sF = sF - (float)(cF + 1);
+        const float frF = idm_free(vF, v0F);
+        const float aF_new = idm_follow(p, a_F_, Kinv_F, frF, vF, s_lag, vF - v);                       // G3
+        const float a_F = has_Lt ? idm_follow(p, a_F_, Kinv_F, frF, vF, sF, vF - vLt) : a_F_ * frF;
+        at_c = has_Lt ? idm_follow(p, a_i, Kinv_i, fr, v, s_Lt, v - vLt) : acc_free;
+        const float a_c = lead_on_edge ? acc_follow : acc_free;
+        const bool ok = (!has_Lt || s_Lt >= p.s0) &&                                                   // G1
+                        (!has_F || (s_lag >= p.s0 && s_lag >= m && aF_new >= -p.b_safe));              // G2, G3
+        const float rem = Cf - x;                                                                      // G4
+        float inc = at_c - a_c;
+        if (has_F) {
+            float d2 = aF_new - a_F;
+            d2 = p.politeness * d2;
+            inc = inc + d2;
         }
-        if (ok && has_F) {                                                   // G3
-            aF_new = idm(p, a_F_, Kinv_F, vF, v0F, true, s_lag, vF - v);
-            ok = aF_new >= -p.b_safe;
-        }
-        if (ok) {                                                            // G4
-            const float rem = Cf - x;
-            at_c = idm(p, a_i, Kinv_i, v, v0, has_Lt, s_Lt, v - vLt);
-            if (!last && l >= lanes2 && lt < l && rem <= mand) accepted = true;
-            else if (!last && lt >= lanes2 && rem <= mand) accepted = false;
-            else {
-                const float a_c = idm(p, a_i, Kinv_i, v, v0, lead_on_edge, s_lead, dv_lead);
-                float inc = at_c - a_c;
-                if (has_F) {
-                    float sF = (float)cLt - len_Lt;
-                    sF = sF - (float)(cF + 1);
-                    const float a_F = idm(p, a_F_, Kinv_F, vF, v0F, has_Lt, sF, vF - vLt);
-                    float d2 = aF_new - a_F;
-                    d2 = p.politeness * d2;
-                    inc = inc + d2;
-                }
-                accepted = inc > p.lc_threshold;
-            }
-        }
+        const bool inside = !last && rem <= mand;
+        const bool mandatory = inside && l >= lanes2 && lt < l;
+        const bool veto = inside && lt >= lanes2;
+        accepted = ok && (mandatory || (!veto && inc > p.lc_threshold));
+        if (!has_Lt) s_Lt = 0.0f;
     }
 
-    // 2e acceleration (min over leader, stop line, new-lane leader) and integration (E2)
-    float acc = idm(p, a_i, Kinv_i, v, v0, has_lead, s_lead, dv_lead);
-    if (!may_cross) acc = fminf(acc, idm(p, a_i, Kinv_i, v, v0, true, Cf - x, v));             // 2c
+    // 2e integration (E2)
     float cap = __int_as_float(0x7f800000);
     if (has_lead) cap = fmaxf(s_lead, 0.0f);
     if (accepted && has_Lt) { acc = fminf(acc, at_c); cap = fminf(cap, fmaxf(s_Lt, 0.0f)); }
