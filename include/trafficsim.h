@@ -160,8 +160,8 @@ typedef struct ts_state_out {
     uint64_t vehicle_updates; /* sum over steps of ACTIVE vehicles advanced (the bench metric) */
 } ts_state_out;
 
-/* Length-E integer accumulators (PAPER.md:437 samples; PAPER.md:446 utilisation is derived
- * on the host: sample_count_sum / n_samples / (len * lanes / (veh_len + s0))). */
+/* Length-E integer accumulators (PAPER.md:437 samples; the utilisation of PAPER.md:446 is derived
+ * from them by ts_read_utilisation). */
 typedef struct ts_edge_stats_out {
     uint32_t *entered;               /* vehicles that entered the edge (departures included) */
     uint32_t *exited;                /* vehicles that left it (arrivals included) */
@@ -177,12 +177,25 @@ typedef struct ts_sim ts_sim;
 int ts_query_workspace(const ts_network *net, const ts_routes *routes,
                        const ts_departures *dep, const ts_params *params, size_t *bytes);
 
-/* Validate, lay out the workspace, copy the inputs (H2D on dev->cuda_stream) and set the
- * state of step 0: every vehicle PENDING, atlas empty.  *out is NULL on failure. */
+/* The inputs of the microsimulation, PAPER.md:366-374 ("the road network ... each edge contains the
+ * number of lanes, the speed limit", per-vehicle departure times and procedural variables) and
+ * PAPER.md:382-384 (the per-vehicle paths): validate them, lay out the workspace, copy them (H2D on
+ * dev->cuda_stream) and set the state of step 0: every vehicle PENDING, the traffic atlas of
+ * PAPER.md:404-406 empty.  All pointers inside the structs are HOST pointers owned by the caller; the
+ * library copies what it needs and keeps none.  *out is NULL on failure.
+ * Errors: TS_EINVAL (sizes, ranges, a route that is not contiguous, look-ahead or entry zone shorter
+ * than one step's advance, signal cycle beyond 2^24 steps, ...), TS_ENOMEM (workspace smaller than
+ * ts_query_workspace says), TS_ECUDA (no device: there is no CPU fallback). */
 int ts_create(const ts_network *net, const ts_routes *routes, const ts_departures *dep,
               const ts_params *params, const ts_device *dev, ts_sim **out);
 
-/* Enqueue n steps (one step = DESIGN.md section 2, steps 1-5).  Asynchronous. */
+/* The time-stepped simulation of PAPER.md:390 ("we simulate the traffic by updating each individual
+ * vehicle: lane changing (mandatory or discretionary) and vehicle following, and update the travel
+ * time, position, and velocity ... In our implementation, we use dt = 0.5 s"): enqueue n steps on the
+ * stream (one step = DESIGN.md section 2, steps 1-5: signals, intent of every ACTIVE vehicle by Eq. 7
+ * PAPER.md:394-397 and the lane-change / gap-acceptance rules PAPER.md:399-400, departures, claims at
+ * the controls of PAPER.md:402, commit, sampling).  Asynchronous; returns TS_EINVARIANT if a sticky
+ * device error was read back earlier, TS_EINVAL if the step counter would pass 2^31. */
 int ts_step(ts_sim *sim, uint32_t n);
 
 /* Same, and writes one 64-bit state digest per step to digests[0..n) (DESIGN.md section 2.6:
@@ -193,9 +206,28 @@ int ts_step_digest(ts_sim *sim, uint32_t n, uint64_t *digests);
 /* Back to step 0 without re-uploading the inputs. */
 int ts_reset(ts_sim *sim);
 
-/* Snapshot in vehicle-id order.  Synchronises; reports the sticky TS_EINVARIANT if raised. */
+/* Per-vehicle outputs, PAPER.md:360 ("Given we simulate individual vehicles, we can extract many
+ * measurements"): a snapshot in vehicle-id order into caller-allocated arrays (HOST pointers unless
+ * ts_device.out_on_device; any may be NULL) plus scalars.  Runs the device-side audit of the atlas
+ * (every ACTIVE vehicle's cell is marked, exactly n_active cells are marked, no position or speed is
+ * NaN, negative or infinite) and reports a violation as the sticky TS_EINVARIANT.  Synchronises. */
 int ts_read_state(ts_sim *sim, ts_state_out *out);
+
+/* Per-edge outputs, PAPER.md:437 ("we sample every minute the utilization and per edge speed"): the
+ * integer accumulators since ts_create / ts_reset / the last call with reset != 0 (which zeroes them
+ * after the copy).  Length-E caller-allocated arrays (HOST unless out_on_device; any may be NULL).
+ * Synchronises. */
 int ts_read_edge_stats(ts_sim *sim, ts_edge_stats_out *out, int reset);
+
+/* "We defined utilization as the number of vehicles at the sampling time divided by the
+ * maximum number of vehicles that can fit on the edge.  This capacity is computed as the length of the
+ * edge times the number of lines divided by the average length of a vehicle plus the lead gap" --
+ * utilisation[e] = (sample_count_sum[e] / n_samples) / (len_e * lanes_e / (veh_len + s0)) -- and the
+ * mean sampled speed in m/s, over the samples since the last reset of the statistics
+ * (reset them every 720 steps for the paper's 6-minute groups).  fp32, computed on the device; two
+ * length-E arrays (HOST unless out_on_device; either may be NULL); 0 where there is no sample.
+ * Synchronises. */
+int ts_read_utilisation(ts_sim *sim, float *utilisation, float *mean_speed);
 
 /* Section 6.3.4 "Vehicle energy consumption and pollution estimates".
  * Fills two caller-allocated length-V fp32 arrays in vehicle-id order (either may be NULL; HOST

@@ -196,3 +196,17 @@ def fuel_rate(v, acc):
 
 def idm(params, v, v0, has_leader, s, dv):
     return float(lib().orc_idm(C.byref(make_params(params)), v, v0, int(has_leader), s, dv))
+
+
+def utilisation(edge_stats, bundle):
+    """"the number of vehicles at the sampling time divided by the maximum number of
+    vehicles that can fit on the edge ... the length of the edge times the number of lines divided by
+    the average length of a vehicle plus the lead gap" (vehicle length of type 0, lead gap s0), averaged
+    over the samples taken; and the mean sampled speed in m/s.  fp64."""
+    p = bundle["params"]
+    cap = bundle["edge_len_m"].astype(np.float64) * bundle["edge_lanes"] / (p["veh_len"] + p["s0"])
+    n = int(edge_stats["n_samples"])
+    cnt = edge_stats["sample_count_sum"].astype(np.float64)
+    util = cnt / n / cap if n else np.zeros_like(cap)
+    speed = np.where(cnt > 0, edge_stats["sample_speedcode_sum"] * 0.25 / np.maximum(cnt, 1), 0.0)
+    return util, speed

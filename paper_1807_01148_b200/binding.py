@@ -17,7 +17,7 @@ TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
            "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile",
-           "ts_read_emissions", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_destroy", "ts_last_error", "ts_version"]
+           "ts_read_emissions", "ts_read_utilisation", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_destroy", "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -124,7 +124,8 @@ def load():
         L.ts_version.restype = C.c_char_p
         L.ts_sue_workspace.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         L.ts_sue_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        for n in EXPORTS[:14]:
+        L.ts_read_utilisation.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        for n in EXPORTS[:15]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -218,6 +219,12 @@ class Sim:
                    vehicle_updates=o.vehicle_updates)
         return out
 
+    def read_utilisation(self):
+        """ts_read_utilisation: per-edge utilisation and mean sampled speed."""
+        u, v = np.zeros(self.E, np.float32), np.zeros(self.E, np.float32)
+        _check(load().ts_read_utilisation(self._h, u.ctypes.data, v.ctypes.data))
+        return u, v
+
     def reroute(self, w_free, mask=None):
         """ts_reroute: new routes for the masked vehicles from the edge statistics accumulated so far
         (PAPER.md:386); resets the simulation.  Returns counts, device times and the weights used."""
@@ -285,15 +292,6 @@ class Sim:
             self.close()
         except Exception:
             pass
-
-
-def utilisation(edge_stats, bundle):
-    """vehicles on the edge at the sampling time divided by the number that fit:
-    length x lanes / (vehicle length + lead gap), averaged over the samples taken."""
-    p = bundle["params"]
-    cap = bundle["edge_len_m"].astype(np.float64) * bundle["edge_lanes"] / (p["veh_len"] + p["s0"])
-    n = max(1, int(edge_stats["n_samples"]))
-    return edge_stats["sample_count_sum"] / n / cap
 
 
 def sue_solve(n_nodes, edge_from, edge_to, t0, cap, od_origin, od_dest, od_trips, iterations=20, bisections=40,

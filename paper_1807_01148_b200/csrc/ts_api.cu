@@ -115,7 +115,7 @@ struct Layout {
         o_status = take(V); o_lane = take(V);
         o_edge = take((size_t)V * 4); o_x = take((size_t)V * 4); o_v = take((size_t)V * 4);
         o_rpos = take((size_t)V * 4); o_insert = take((size_t)V * 4); o_arrive = take((size_t)V * 4);
-        o_cell = take((size_t)V * 4); o_ridx = take((size_t)V * 4);
+        o_cell = take((size_t)std::max(V, E) * 4); o_ridx = take((size_t)std::max(V, E) * 4);   // read-back scratch (per vehicle or per edge)
         st_entered = take((size_t)E * 4); st_exited = take((size_t)E * 4);
         st_exit_steps = take((size_t)E * 8); st_samp_cnt = take((size_t)E * 4);
         st_samp_code = take((size_t)E * 8);
@@ -474,7 +474,9 @@ __global__ void k_audit(const __grid_constant__ Ctx c, uint32_t cur, size_t n_wo
     for (size_t s = tid; s < n_slots; s += nthreads) {
         const uint4 sa = c.s[cur].A[s];
         if (!(sa.w & ALIVE)) continue;
-        const uint32_t gc = (sa.z << 7) + (uint32_t)(int)floorf(__uint_as_float(sa.x));
+        const float xs = __uint_as_float(sa.x), vs = __uint_as_float(sa.y);
+        if (!(xs >= 0.0f) || !(vs >= 0.0f) || isinf(xs) || isinf(vs)) { atomicOr(&c.dyn->error, ERR_NAN); continue; }   // NaN, negative or infinite
+        const uint32_t gc = (sa.z << 7) + (uint32_t)(int)floorf(xs);
         if (!((occ32[gc >> 5] >> (gc & 31)) & 1u)) missing++;
     }
     for (int o = 16; o; o >>= 1) {
@@ -1055,6 +1057,7 @@ static int copy_out(ts_sim* s, void* dst, const void* src, size_t bytes) {
 static const char* describe(uint32_t err) {
     if (err & ERR_CELL_CLASH) return "atlas audit failed: two vehicles in one lane cell, or a vehicle whose cell is not marked";
     if (err & ERR_SLOTS) return "slot overflow";
+    if (err & ERR_NAN) return "a vehicle's position or speed is NaN, negative or infinite";
     return "internal logic check failed";
 }
 
@@ -1156,6 +1159,33 @@ extern "C" int ts_read_edge_stats(ts_sim* s, ts_edge_stats_out* o, int reset) {
         CUDA_TRY(cudaMemsetAsync(s->ws + L.st_entered, 0, L.emis - L.st_entered, s->stream));
         CUDA_TRY(cudaMemsetAsync(s->ws + L.dyn + offsetof(Dyn, n_samples), 0, 4, s->stream));
     }
+    return TS_OK;
+}
+
+// "We defined utilization as the number of vehicles at the sampling time divided by the
+// maximum number of vehicles that can fit on the edge.  This capacity is computed as the length of the
+// edge times the number of lines divided by the average length of a vehicle plus the lead gap" -- and the
+// per-edge speed of PAPER.md:437, both averaged over the samples taken since the last reset.
+__global__ void k_utilisation(const __grid_constant__ Ctx c, float* util, float* speed) {
+    const uint32_t n_samples = c.dyn->n_samples;
+    for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < c.E; e += gridDim.x * blockDim.x) {
+        const EdgeRec E = c.edges[e];
+        const float cap = ((float)E.len * (float)edge_lanes(E)) / (c.p.len + c.p.s0);
+        const uint32_t cnt = c.st_samp_cnt[e];
+        util[e] = n_samples ? ((float)cnt / (float)n_samples) / cap : 0.0f;
+        speed[e] = cnt ? ((float)c.st_samp_code[e] * 0.25f) / (float)cnt : 0.0f;
+    }
+}
+
+extern "C" int ts_read_utilisation(ts_sim* s, float* utilisation, float* mean_speed) {
+    if (!s) return fail(TS_EINVAL, "null sim");
+    Layout& L = s->L;
+    k_utilisation<<<std::max(1u, std::min(1184u, (L.E + 255) / 256)), 256, 0, s->stream>>>(s->ctx, at<float>(s, L.o_cell), at<float>(s, L.o_ridx));
+    CUDA_TRY(cudaGetLastError());
+    int rc = 0;
+    if ((rc = copy_out(s, utilisation, s->ws + L.o_cell, (size_t)L.E * 4))) return rc;
+    if ((rc = copy_out(s, mean_speed, s->ws + L.o_ridx, (size_t)L.E * 4))) return rc;
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
     return TS_OK;
 }
 

@@ -34,7 +34,7 @@ constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 // CTRL_STOP: stop control with a persistent node owner (reading R34); CTRL_SIGNAL_NM:
 // one signal phase per movement (inbound edge, outbound edge) ("combination nm"; R35)
 enum : uint32_t { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2, CTRL_STOP = 3, CTRL_SIGNAL_NM = 4 };
-enum : uint32_t { ERR_CELL_CLASH = 1, ERR_SLOTS = 2, ERR_LOGIC = 4 };
+enum : uint32_t { ERR_CELL_CLASH = 1, ERR_SLOTS = 2, ERR_LOGIC = 4, ERR_NAN = 8 };
 // flags in Slots::A.w above the lane number: the vehicle takes part in the steps; has made its stop
 // at the STOP line of its edge; holds the STOP node at the tail of its edge; its type
 enum : uint32_t { ALIVE = 0x100u, STOPPED = 0x200u, OWNS = 0x400u, TYPE_SHIFT = 12, TYPE_MASK = 0x3000u };

@@ -109,3 +109,21 @@ def test_multi_step_digests_with_many_slots_per_thread():
         assert bad.size == 0, f"first digest mismatch at step {int(bad[0]) + 1} of the call"
     assert sim.read_counts()["n_active"] > 9472 * 10          # more than 10 slots per thread
     sim.close()
+
+
+def test_utilisation_and_sampled_speed(cfg1):
+    """ts_read_utilisation against the oracle's fp64 arithmetic on the same
+    integer samples (fp32 on the device: 1e-6 relative), and its reset semantics."""
+    import paper_1807_01148_b200 as pkg
+    from oracle import Oracle, utilisation
+    b = small_signal_grid()
+    orc, sim = Oracle(b), pkg.Sim(b, "cuda:0")
+    orc.step(1300); sim.step(1300)
+    u, v = sim.read_utilisation()
+    wu, wv = utilisation(orc.read_edge_stats(), b)
+    assert wu.max() > 0.05
+    assert np.allclose(u, wu, rtol=2e-6, atol=1e-9) and np.allclose(v, wv, rtol=2e-6, atol=1e-9)
+    sim.read_edge_stats(reset=True)
+    u, v = sim.read_utilisation()
+    assert not u.any() and not v.any()
+    sim.close()

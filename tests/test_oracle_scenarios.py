@@ -142,3 +142,27 @@ def test_departures_are_fifo_by_step_then_id_and_wait_for_a_clear_entry():
     # takes several steps, so consecutive entries are > 1 step apart while the queue is backed up
     backed_up = dep_step[order][1:] + 1 < ins[1:]
     assert backed_up.any() and (np.diff(ins)[backed_up] >= 5).all()
+
+
+def test_utilisation_of_a_jammed_edge_is_one():
+    """PAPER.md:446 defines utilisation against the number of vehicles that fit, length x lanes /
+    (vehicle length + lead gap).  A one-lane edge behind a permanently red light fills up with a
+    standing queue at veh_len + s0 = 7 m spacing (pin P3), so its sampled utilisation must come out
+    at 1 (+- one vehicle), and its sampled speed at 0; the empty edge beyond the light at 0."""
+    from oracle import utilisation
+    N = 3
+    sig = (np.full(N, 1), np.full(N, 1_000_000), np.full(N, 1))
+    b = corridor(n_edges=2, length=210, departs=np.arange(60) * 3.0, ctrl=W.CTRL_SIGNAL, sig=sig, steps=3000)
+    o = Oracle(b)
+    o.step(2400)                      # the queue has filled the edge
+    o.read_edge_stats(reset=True)
+    o.step(600)                       # five samples of the standing queue
+    es = o.read_edge_stats()
+    util, speed = utilisation(es, b)
+    assert es["n_samples"] == 5
+    assert abs(util[0] - 1.0) <= 7.0 / 210 + 1e-9 and util[1] == 0.0
+    assert speed[0] < 0.05
+    # by hand: 14 vehicle-samples over 2 samples on 100 m x 2 lanes -> 7 / (200 / 7)
+    es2 = dict(sample_count_sum=np.array([14]), sample_speedcode_sum=np.array([14 * 40]), n_samples=2)
+    u2, v2 = utilisation(es2, dict(b, edge_len_m=np.array([100]), edge_lanes=np.array([2])))
+    assert u2[0] == 7.0 / (200.0 / 7.0) and v2[0] == 10.0
