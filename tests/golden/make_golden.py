@@ -21,6 +21,10 @@ Stored per config (nothing here ever comes from the CUDA path):
   (--emissions: a separate file emissions_<cfg>.json with the whole-run totals of the section
              6.3.4 accumulators: per array the fp64 sum, the sum of the fp32 bit
              patterns and a position-weighted sum of the bit patterns, plus the final digest)
+  final_state (written with the last mark) per array of the oracle's read_state -- status, edge, lane,
+             route_idx, insert_step, arrive_step and the bit patterns of x and v, all V vehicles in id
+             order -- its sum and a position-weighted checksum: what the digests (ACTIVE vehicles only) do
+             not cover
   complete   false while the run is in progress: the file is rewritten after every stride, so an
              interrupted run of a very long config (config 4: 5.4e10 vehicle-updates, many hours of
              the single-threaded oracle) still leaves a usable prefix of digests
@@ -39,6 +43,17 @@ sys.path.insert(0, ROOT)
 
 from oracle import Oracle                                    # noqa: E402
 from paper_1807_01148_b200 import workload as W              # noqa: E402
+
+
+def state_checksums(st):
+    """Sum and position-weighted checksum of every per-vehicle array of a read_state() dict."""
+    out = {}
+    for k in ("status", "edge", "lane", "route_idx", "insert_step", "arrive_step", "x", "v"):
+        a = np.asarray(st[k])
+        u = (a.view(np.uint32) if a.dtype == np.float32 else a).astype(np.uint64)
+        w = np.arange(1, len(u) + 1, dtype=np.uint64)
+        out[k] = [int(u.sum()), int((u * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF))]
+    return out
 
 
 def run(name, stride, suffix="", threads=1):
@@ -72,6 +87,8 @@ def run(name, stride, suffix="", threads=1):
                    final=dict(n_pending=int(counts["n_pending"]), n_active=int(counts["n_active"]),
                               n_arrived=int(counts["n_arrived"])),
                    seconds=round(time.perf_counter() - t0, 1), threads=threads)
+        if done == steps:
+            out["final_state"] = state_checksums(orc.read_state())
         with open(path + ".tmp", "w") as f:
             json.dump(out, f, indent=1)
         os.replace(path + ".tmp", path)

@@ -22,7 +22,7 @@ def test_script_reproduces_the_committed_config1_trace(tmp_path, monkeypatch):
     mod.run("cfg1", 600)
     new = json.load(open(tmp_path / "trace_cfg1.json"))
     old = json.load(open(os.path.join(GOLDEN, "trace_cfg1.json")))
-    for key in ("sha256", "steps", "marks", "digests", "active", "counters", "final", "edge_stats"):
+    for key in ("sha256", "steps", "marks", "digests", "active", "counters", "final", "edge_stats", "final_state"):
         assert new[key] == old[key], key
     assert new["complete"] and new["marks"][-1] == new["steps"] == 3600
     assert new["final"] == dict(n_pending=0, n_active=0, n_arrived=500)

@@ -61,11 +61,19 @@ def test_full_run_matches_golden_digests(name):
             v = np.asarray(es[key], np.uint64)
             assert int(v.sum()) == total, key
             assert int((v * w).sum() & np.uint64(0xFFFFFFFFFFFFFFFF)) == weighted, key
+    if "final_state" in tr:                 # every vehicle's final record, PENDING and ARRIVED ones included
+        import importlib.util
+        spec = importlib.util.spec_from_file_location("make_golden", os.path.join(GOLDEN, "make_golden.py"))
+        mg = importlib.util.module_from_spec(spec)
+        spec.loader.exec_module(mg)
+        got_state = mg.state_checksums(sim.read_state())
+        for key, pair in tr["final_state"].items():
+            assert got_state[key] == pair, f"final {key}"
     assert np.all(np.diff(tr["marks"]) > 0)
     sim.close()
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5", "cfg3"])
 def test_full_run_emission_totals(name):
     """Section 6.3.4 at full size, default launch configuration, WHOLE run: the
     oracle's per-vehicle CO and fuel totals are stored as checksums of their fp32 bit patterns
