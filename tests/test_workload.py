@@ -53,3 +53,27 @@ def test_config3_and_5_small():
     b5 = W.config5(n_vehicles=2000, grid=16, steps=100, core=4, workers=2)
     _check_bundle(b5)
     assert len(np.unique(b5["edge_from"][b5["route_edges"][b5["route_off"][:-1].astype(np.int64)]])) <= 16
+
+
+def test_variant_helpers_keep_the_demand_and_only_add_inputs():
+    """with_trucks / with_controls, the re-routing inputs (row 1) and the
+    static-assignment inputs (row 5) are derived from a config without touching its network or routes."""
+    b = W.config1()
+    t = W.with_trucks(b, share=0.3)
+    assert t["veh_type"].dtype == np.uint8 and 0.2 < t["veh_type"].mean() < 0.4
+    assert t["params"]["n_types"] == 2 and np.array_equal(t["route_edges"], b["route_edges"])
+    assert W.bundle_sha256(t) != W.bundle_sha256(b)
+    c = W.with_controls(b, amber_steps=4)
+    assert (c["node_ctrl"] == W.CTRL_STOP).all() and c["params"]["amber_steps"] == 4
+    c2 = W.with_controls(W.config2(n_vehicles=10))
+    assert set(np.unique(c2["node_ctrl"])) == {W.CTRL_SIGNAL, W.CTRL_SIGNAL_NM}
+    wf = W.free_flow_weights(b)
+    assert wf.dtype == np.uint32 and (wf >= 1).all() and (wf <= 1 << 20).all()
+    # 200 m at 15 m/s on 2 lanes: 200 / (15 sqrt 2) s = 18.86 steps of 0.5 s = 4827 units of 1/256 step
+    assert wf[0] == round(200 / (15 * 2 ** 0.5) / 0.5 * 256)
+    shares = [W.reroute_mask(100000, it).mean() for it in range(4)]
+    assert shares[0] == shares[1] == 1.0 and abs(shares[2] - 0.5) < 0.01 and abs(shares[3] - 0.25) < 0.01
+    assert np.array_equal(W.reroute_mask(1000, 2), W.reroute_mask(1000, 2))             # seeded
+    s = W.sue_inputs(b, horizon_s=60.0)
+    assert int(s["od_trips"].sum()) == b["n_vehicles"] and (s["od_origin"] != s["od_dest"]).all()
+    assert np.allclose(s["t0"], 200 / 15.0) and np.allclose(s["cap"], 900.0 * 2 / 3600.0 * 60.0)
