@@ -474,6 +474,38 @@ def with_controls(bundle, seed=0, amber_steps=6, name=None):
                 params=dict(bundle["params"], amber_steps=amber_steps, stop_dist=4.0, stop_speed=0.5))
 
 
+# --------------------------------------------------------------------------- edge numbering
+
+def spatial_edge_order(bundle, bits=16):
+    """A space-filling (Morton / Z-curve) order of the edges by the midpoint of their end nodes:
+    order[new id] = old id.  The simulator lays out edge records, atlas rows and claim words in the
+    CALLER's edge order, so an edge numbering with spatial locality is what keeps a metro-scale network's
+    gathers in L2 (config 4)."""
+    xy = np.asarray(bundle["node_xy"], np.float64)
+    mid = 0.5 * (xy[bundle["edge_from"]] + xy[bundle["edge_to"]])
+    lo, hi = mid.min(0), mid.max(0)
+    q = np.minimum(((mid - lo) / np.maximum(hi - lo, 1e-9) * (1 << bits)).astype(np.uint64), (1 << bits) - 1)
+    code = np.zeros(len(mid), np.uint64)
+    for k in range(bits):
+        code |= ((q[:, 0] >> np.uint64(k)) & np.uint64(1)) << np.uint64(2 * k)
+        code |= ((q[:, 1] >> np.uint64(k)) & np.uint64(1)) << np.uint64(2 * k + 1)
+    return np.argsort(code, kind="stable").astype(np.uint32)
+
+
+def renumber_edges(bundle, order, name=None):
+    """The same network and demand with edge `order[n]` renamed `n` (edge arrays permuted, routes
+    translated).  A different input as far as the simulators are concerned: ties that go by edge index
+    (signal phase order, R16 / R35) fall differently, so its results are its own."""
+    order = np.asarray(order, np.int64)
+    new_id = np.empty(len(order), np.uint32)
+    new_id[order] = np.arange(len(order), dtype=np.uint32)
+    out = dict(bundle, name=name or bundle["name"] + "_renumbered")
+    for k in ("edge_from", "edge_to", "edge_len_m", "edge_lanes", "edge_vlim"):
+        out[k] = np.ascontiguousarray(bundle[k][order])
+    out["route_edges"] = new_id[bundle["route_edges"]]
+    return out
+
+
 # --------------------------------------------------------------------------- re-routing inputs
 
 REROUTE_SHARES = (1.0, 1.0, 0.5, 0.25)     # PAPER.md:386: "all routes the first and second iteration, and
@@ -525,6 +557,10 @@ def sue_inputs(bundle, horizon_s=3600.0):
 _BY_NAME = {
     "cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5,
     "cfg3_dense": config3_dense,
+    # config 4's network and demand with its edges numbered along a space-filling curve (diagnostic: DESIGN.md section 6)
+    "cfg4_morton": lambda: (lambda b: renumber_edges(b, spatial_edge_order(b), "cfg4_metro_morton"))(config4()),
+    "cfg4_small_morton": lambda: (lambda b: renumber_edges(b, spatial_edge_order(b), "cfg4_small_morton"))(
+        config4(n_vehicles=60_000, steps=7200, n_points=20_000, side_m=14_000.0, n_centroids=256, name="cfg4_small")),
     # SURVEY.md 8(f) rows 3 and 4 on config 2's network and demand
     "cfg2_trucks": lambda: with_trucks(config2()),
     "cfg2_controls": lambda: with_controls(config2()),

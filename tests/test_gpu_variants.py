@@ -127,3 +127,12 @@ def test_utilisation_and_sampled_speed(cfg1):
     u, v = sim.read_utilisation()
     assert not u.any() and not v.any()
     sim.close()
+
+
+def test_renumbered_edges_morton_order():
+    """workload.renumber_edges / spatial_edge_order: the same network with its edges numbered along a
+    space-filling curve is a different input (ties by edge index fall differently) and must match the
+    oracle run on THAT input, bit for bit."""
+    b = W.by_name("cfg4_small_morton")
+    assert b["name"] == "cfg4_small_morton"
+    _compare(b, 7200, 1, chunk=3600)
