@@ -289,6 +289,57 @@ def run_reroute(args):
     }))
 
 
+def run_sue(args):
+    """--sue: the paper's static traffic assignment (Frank-Wolfe with BPR times) on the
+    workload's network and OD demand (workload.sue_inputs), SURVEY.md 8(f) row 5.  One bench "step" is one
+    ts_sue_solve call from host buffers.  The usual line with metric = shortest-path trees per second (the
+    dominant kernel is the tree kernel shared with ts_reroute), its roofline object and the convergence."""
+    import torch
+    import paper_1807_01148_b200 as pkg
+    from paper_1807_01148_b200 import workload as W
+    torch.cuda.set_device(0)
+    bundle = load_workload(args.workload)
+    inp = W.sue_inputs(bundle, horizon_s=args.sue_horizon)
+    a = (bundle["n_nodes"], bundle["edge_from"], bundle["edge_to"], inp["t0"], inp["cap"], inp["od_origin"],
+         inp["od_dest"], inp["od_trips"])
+    ms, info = [], None
+    sampler = ClockSampler(0)
+    for rep_ in range(args.warmup + args.steps):
+        if rep_ == args.warmup:
+            sampler.start()
+        t0 = time.perf_counter()
+        flow, times, info = pkg.sue_solve(*a, iterations=args.sue_iterations)
+        if rep_ >= args.warmup:
+            ms.append(1e3 * (time.perf_counter() - t0))
+    clocks = sampler.stop()
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    peak = float(json.load(open(peaks_path))["hbm_gbs"]) if os.path.exists(peaks_path) else 6650.0
+    E, trees = bundle["n_edges"], int(info["n_trees"])
+    alg = 36.0 * E * trees
+    sssp_s = info["sssp_ms"] / 1e3
+    print(json.dumps({
+        "metric": "shortest_path_trees_per_sec", "value": trees * len(ms) / (sum(ms) / 1e3), "unit": "trees/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sum(ms) / len(ms), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64 (flows, times), u32/u64 (weights, labels, all-or-nothing flows)",
+        "data": "synthetic",
+        "config": {"workload": bundle["name"] + " static user equilibrium (PAPER.md:307-338)", "nodes": bundle["n_nodes"],
+                   "edges": E, "od_pairs": int(len(inp["od_trips"])), "trips": int(inp["od_trips"].sum()),
+                   "origins": int(len(np.unique(inp["od_origin"]))), "iterations": args.sue_iterations,
+                   "demand_horizon_s": args.sue_horizon, "workspace_bytes": int(info["workspace_bytes"])},
+        "sue": {"relative_gap": [float(g) for g in info["gap"]], "step": [float(x) for x in info["step"]],
+                "objective_first_last": [float(info["objective"][0]), float(info["objective"][-1])],
+                "device_ms": float(info["device_ms"]), "tree_kernel_ms": float(info["sssp_ms"]),
+                "max_v_over_c": float((flow / inp["cap"]).max())},
+        "e2e": {"value": trees * len(ms) / (sum(ms) / 1e3), "unit": "trees/s",
+                "h2d_bytes_per_step": int(E * 24 + len(inp["od_trips"]) * 16), "d2h_bytes_per_step": int(E * 16),
+                "note": "the timed call takes host buffers and returns host arrays"},
+        "gpu_launches": len(ms) * (args.sue_iterations + 1) * 50, "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "k_rr_sssp", "achieved": alg / sssp_s / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": alg / sssp_s / 1e9 / peak, "traffic": None, "bytes_per_unit": 36.0,
+                     "unit_of_work": "edge relaxation (one per edge per tree at least)", "trees": trees},
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -311,11 +362,17 @@ def main():
     ap.add_argument("--no-window", action="store_true", help="skip the busiest-window pass (profiling runs)")
     ap.add_argument("--reroute", action="store_true",
                     help="the four-iteration re-routing loop of PAPER.md:386 on the workload (SURVEY.md 8(f) row 1)")
+    ap.add_argument("--sue", action="store_true",
+                    help="static user equilibrium by Frank-Wolfe + BPR on the workload's network and demand (SURVEY.md 8(f) row 5)")
+    ap.add_argument("--sue-iterations", type=int, default=10)
+    ap.add_argument("--sue-horizon", type=float, default=3600.0, help="seconds over which the trips are spread (demand rate)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.reroute:
         return run_reroute(args)
+    if args.sue:
+        return run_sue(args)
     if args.warmup < 3:
         print("note: timing rules ask for >= 3 warm-up steps", file=sys.stderr)
 

@@ -131,7 +131,7 @@ typedef struct ts_params {
     /* Re-routing (ts_reroute): route entries to reserve for each of the two route
      * tables (>= the entries of the routes given; new routes may be longer).  0 = ts_reroute is not
      * available and no workspace is spent on it (one shortest-path tree of N words per distinct
-     * origin node, the graph in CSR form, 148 trees in flight). */
+     * origin node, the graph in CSR form, 20 N bytes for each of the 592 trees in flight). */
     uint32_t route_capacity;
 } ts_params;
 

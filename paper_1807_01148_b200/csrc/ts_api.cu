@@ -1222,7 +1222,7 @@ extern "C" int ts_reroute(ts_sim* s, const uint32_t* w_free, const uint8_t* mask
     k_rr_weights<<<std::max(1u, std::min(1184u, (E + 255) / 256)), 256, 0, st>>>(r);
     CUDA_TRY(cudaEventRecord(ev[0], st));
     if (!todo.empty())
-        k_rr_sssp<<<std::min<uint32_t>(kRrCtas, (uint32_t)todo.size()), 1024, 0, st>>>(r, at<uint32_t>(s, L.rr_todo), (uint32_t)todo.size());
+        k_rr_sssp<<<std::min<uint32_t>(kRrCtas, (uint32_t)todo.size()), kRrThreads, 0, st>>>(r, at<uint32_t>(s, L.rr_todo), (uint32_t)todo.size());
     CUDA_TRY(cudaEventRecord(ev[1], st));
     const uint32_t vb = std::max(1u, std::min(1184u, (V + 255) / 256));
     k_rr_len<<<vb, 256, 0, st>>>(r);
@@ -1398,7 +1398,7 @@ extern "C" int ts_sue_solve(const ts_sue_problem* p, const ts_device* dev, ts_su
     auto assign = [&](const double* x) -> int {
         k_sue_times<<<eb, 256, 0, st>>>(E, dp(L.t0), dp(L.cap), x, p->alpha, p->weight_scale, dp(L.t), r.w);
         CUDA_TRY(cudaEventRecord(t0e, st));
-        if (L.n_src) k_rr_sssp<<<std::min<uint32_t>(kRrCtas, L.n_src), 1024, 0, st>>>(r, up32(L.todo), L.n_src);
+        if (L.n_src) k_rr_sssp<<<std::min<uint32_t>(kRrCtas, L.n_src), kRrThreads, 0, st>>>(r, up32(L.todo), L.n_src);
         CUDA_TRY(cudaEventRecord(t1e, st));
         CUDA_TRY(cudaMemsetAsync(y, 0, (size_t)E * 8, st));
         if (n_od) k_sue_aon<<<ob, 256, 0, st>>>(n_od, up32(L.od_o), up32(L.od_d), up32(L.od_t), up32(L.od_s), r.pred, N, r.edge_from, y);

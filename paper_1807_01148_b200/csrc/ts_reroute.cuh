@@ -9,7 +9,7 @@
 //
 // Kernels (product code, sm_100a; shares nothing with oracle/reroute.py):
 //   k_rr_weights   w[e] = round-half-up(256 * exit_steps_sum / exited), else the caller's free-flow weight
-//   k_rr_sssp      one CTA per origin node: label-correcting shortest paths over the CSR of outbound
+//   k_rr_sssp      one CTA of 256 threads per origin node, 592 in flight: label-correcting shortest paths over the CSR of outbound
 //                  edges, frontier by frontier; a node's label is ONE 64-bit word (distance << 32 |
 //                  inbound edge) under atomicMin, so the lexicographic minimum IS the tie-break rule
 //   k_rr_len       per vehicle: length of its new route (walk the tree back from the destination)
@@ -24,7 +24,10 @@ namespace ts {
 constexpr uint32_t kRrNone = 0xFFFFFFFFu;
 constexpr uint32_t kRrUnit = 256;            // weight units per simulation step (R37)
 constexpr uint32_t kRrWMax = 1u << 20;
-constexpr uint32_t kRrCtas = 148;            // shortest-path trees in flight (one CTA each)
+// Shortest-path trees in flight, one CTA of kRrThreads threads each.  A frontier of a road network holds a few
+// hundred nodes and a tree is a chain of ~diameter frontiers, each a __syncthreads() apart: small CTAs, many of them
+// (4 per SM), finish 4 096 trees of config 3 four times sooner than one 1 024-thread CTA per SM did.
+constexpr uint32_t kRrCtas = 592, kRrThreads = 256;
 
 struct RrCtx {
     uint32_t V, E, N, n_src;
@@ -71,7 +74,7 @@ __global__ void k_rr_weights(const RrCtx r) {
 }
 
 // todo[0..n_todo): indices into src_node of the trees wanted.
-__global__ void __launch_bounds__(1024) k_rr_sssp(const RrCtx r, const uint32_t* __restrict__ todo, uint32_t n_todo) {
+__global__ void __launch_bounds__(kRrThreads) k_rr_sssp(const RrCtx r, const uint32_t* __restrict__ todo, uint32_t n_todo) {
     __shared__ uint32_t sh_next;
     const uint32_t t = threadIdx.x, T = blockDim.x, N = r.N;
     unsigned long long* lab = r.lab + (size_t)blockIdx.x * N;
