@@ -306,6 +306,28 @@ typedef struct ts_sue_out {
 int ts_sue_workspace(const ts_sue_problem *problem, size_t *bytes);
 int ts_sue_solve(const ts_sue_problem *problem, const ts_device *dev, ts_sue_out *out);
 
+/* Shortest-path trees WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the tree kernel of ts_reroute / ts_sue_solve
+ * (readings R37-R38) with its scratch -- per tree in flight a 64-bit label, two frontier words and
+ * a stamp per node -- in a file-scope static device array of 20 MiB that every GPU loading this library holds
+ * until the process exits.  Limit: n_nodes <= ts_sssp_static_max_nodes() = 65 536 (beyond it: TS_EINVAL and a
+ * message; use the workspace-based calls).  The call allocates nothing on device or host, copies nothing and
+ * does not synchronise: it enqueues ONE kernel on cuda_stream.
+ * ALL pointers are DEVICE pointers owned by the caller:
+ *   d_out_off [n_nodes+1], d_out_edge [n_edges]   CSR of the outbound edges by tail node (edge ids)
+ *   d_edge_to [n_edges]  head nodes;  d_w [n_edges]  integer weights in 1..2^20
+ *   d_sources [n_sources]  source nodes;  d_pred [n_sources * n_nodes]  OUT: row i = tree of d_sources[i], per
+ *                        node the inbound edge on the shortest path (ties: smallest (distance, edge id)),
+ *                        0xFFFFFFFF at the source and at unreachable nodes
+ *   d_error (nullable)   one word the caller has zeroed; set to 1 if a path cost passed 2^32
+ * The static array is shared by every call on the GPU and keeps the last call's contents (nothing needs
+ * clearing: the kernel initialises a tree's labels and stamps before growing it).  Calls that OVERLAP on the GPU
+ * (two streams without a dependency) race on it: order them. */
+uint32_t ts_sssp_static_max_nodes(void);
+int ts_sssp_static(uint32_t n_nodes, uint32_t n_edges, const uint32_t *d_out_off, const uint32_t *d_out_edge,
+                   const uint32_t *d_edge_to, const uint32_t *d_w, const uint32_t *d_sources, uint32_t n_sources,
+                   uint32_t *d_pred, uint32_t *d_error, void *cuda_stream);
+
 /* Tuning knobs that never change results.
  *  "mode"          1 (default) = ts_step(n) is ONE persistent cooperative kernel looping over
  *                  the n steps with grid-wide barriers; 0 = one launch per phase.

@@ -17,7 +17,7 @@ TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
            "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile",
-           "ts_read_emissions", "ts_read_utilisation", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_destroy", "ts_last_error", "ts_version"]
+           "ts_read_emissions", "ts_read_utilisation", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_sssp_static", "ts_sssp_static_max_nodes", "ts_destroy", "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -122,6 +122,9 @@ def load():
         L.ts_destroy.restype = None
         L.ts_last_error.restype = C.c_char_p
         L.ts_version.restype = C.c_char_p
+        L.ts_sssp_static.argtypes = [C.c_uint32, C.c_uint32] + [C.c_void_p] * 5 + [C.c_uint32] + [C.c_void_p] * 3
+        L.ts_sssp_static.restype = C.c_int
+        L.ts_sssp_static_max_nodes.restype = C.c_uint32
         L.ts_sue_workspace.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         L.ts_sue_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.ts_read_utilisation.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -320,3 +323,14 @@ def sue_solve(n_nodes, edge_from, edge_to, t0, cap, od_origin, od_dest, od_trips
     _check(L.ts_sue_solve(C.byref(prob), C.byref(dev), C.byref(out)))
     return flow, time_, dict(objective=obj, gap=gap, step=step, device_ms=out.device_ms, sssp_ms=out.sssp_ms,
                              n_trees=out.n_trees, workspace_bytes=n.value)
+
+
+def sssp_static(n_nodes, out_off, out_edge, edge_to, w, sources, pred, error=None, stream=None):
+    """ts_sssp_static: shortest-path trees with no allocation anywhere (static device scratch, at most
+    ts_sssp_static_max_nodes() nodes).  Every array is a CUDA torch tensor of 32-bit integers the caller
+    owns (`pred`: n_sources * n_nodes words, output); enqueues one kernel on `stream` (default: current)."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(pred.device)
+    ptr = lambda t: None if t is None else t.data_ptr()
+    _check(load().ts_sssp_static(int(n_nodes), int(out_edge.numel()), ptr(out_off), ptr(out_edge), ptr(edge_to),
+                                 ptr(w), ptr(sources), int(sources.numel()), ptr(pred), ptr(error), st.cuda_stream))

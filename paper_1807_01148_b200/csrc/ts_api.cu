@@ -1462,3 +1462,105 @@ extern "C" int ts_sue_solve(const ts_sue_problem* p, const ts_device* dev, ts_su
     if (err) return fail(TS_EINVAL, "a path cost passed 2^32 weight units: lower weight_scale");
     return TS_OK;
 }
+
+// ------------------------------------------------------------------ shortest-path trees without any allocation
+//
+// ts_sssp_static: the tree kernel of ts_reroute / ts_sue_solve for callers that cannot allocate (CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc).  Its scratch -- per tree in flight a 64-bit
+// label, two frontier words and a stamp per node -- lives in ONE file-scope device array of a fixed size, which
+// every GPU that loads this library holds until the process exits.  Nothing here calls cudaMalloc, cudaFree, an
+// allocating library routine or the host allocator; the call only enqueues one kernel on the caller's stream.
+//
+// The array keeps the last call's contents.  Nothing needs clearing between calls: the kernel initialises the
+// labels and stamps of a tree before it grows it, and never reads a frontier slot it did not write.  All calls on
+// one GPU SHARE the array: two calls that overlap on the GPU (different streams, no dependency) race.
+constexpr size_t kStaticScratchBytes = (size_t)20 << 20;          // 20 MiB per GPU
+constexpr uint32_t kStaticMaxNodes = 65536;                        // 20 bytes of scratch per node and tree: 16 trees in flight
+constexpr uint32_t kStaticBytesPerNode = 20;
+static __device__ __align__(256) unsigned char g_sssp_scratch[kStaticScratchBytes];
+
+// Same relaxation as k_rr_sssp (ts_reroute.cuh), trees numbered 0..n_src-1 in the caller's source order;
+// `scratch` is the device address of g_sssp_scratch (device code could name the array directly, the host cannot).
+__global__ void __launch_bounds__(kRrThreads) k_sssp_static(unsigned char* scratch, uint32_t N, const uint32_t* __restrict__ out_off,
+                                                            const uint32_t* __restrict__ out_edge, const uint32_t* __restrict__ edge_to,
+                                                            const uint32_t* __restrict__ w, const uint32_t* __restrict__ sources,
+                                                            uint32_t n_src, uint32_t* __restrict__ pred, uint32_t* error) {
+    __shared__ uint32_t sh_next;
+    const uint32_t t = threadIdx.x, T = blockDim.x, n_cta = gridDim.x;
+    unsigned long long* lab = reinterpret_cast<unsigned long long*>(scratch) + (size_t)blockIdx.x * N;
+    uint32_t* words = reinterpret_cast<uint32_t*>(scratch + (size_t)n_cta * N * 8);
+    uint32_t* fa = words + ((size_t)0 * n_cta + blockIdx.x) * N;
+    uint32_t* fb = words + ((size_t)1 * n_cta + blockIdx.x) * N;
+    uint32_t* stamp = words + ((size_t)2 * n_cta + blockIdx.x) * N;
+    for (uint32_t si = blockIdx.x; si < n_src; si += n_cta) {
+        const uint32_t s = sources[si];
+        for (uint32_t v = t; v < N; v += T) { lab[v] = ~0ull; stamp[v] = 0u; }
+        __syncthreads();
+        if (t == 0) { lab[s] = (unsigned long long)kRrNone; fa[0] = s; sh_next = 0; }
+        __syncthreads();
+        uint32_t n_f = 1, epoch = 0;
+        while (n_f) {
+            epoch++;
+            for (uint32_t i = t; i < n_f; i += T) {
+                const uint32_t u = __ldcg(fa + i);
+                const unsigned long long du = __ldcg(lab + u) >> 32;
+                const uint32_t j1 = out_off[u + 1];
+                for (uint32_t j = out_off[u]; j < j1; j++) {
+                    const uint32_t e = out_edge[j], v = edge_to[e];
+                    const unsigned long long nd = du + w[e];
+                    if (nd >= 0xFFFFFFFFull) { if (error) *error = 1u; continue; }
+                    const unsigned long long cand = (nd << 32) | e;
+                    const unsigned long long old = atomicMin(lab + v, cand);
+                    if (cand < old && nd < (old >> 32) && atomicExch(stamp + v, epoch) != epoch)
+                        fb[atomicAdd(&sh_next, 1u)] = v;
+                }
+            }
+            __syncthreads();
+            n_f = sh_next;
+            __syncthreads();
+            if (t == 0) sh_next = 0;
+            uint32_t* tmp = fa; fa = fb; fb = tmp;
+            __threadfence_block();
+            __syncthreads();
+        }
+        uint32_t* row = pred + (size_t)si * N;
+        for (uint32_t v = t; v < N; v += T) row[v] = (uint32_t)__ldcg(lab + v);
+        __syncthreads();
+    }
+}
+
+// Device address of g_sssp_scratch, resolved once per device with that device current.  In host code the
+// array's NAME is a host-side stand-in, not a device address: only cudaGetSymbolAddress gives the address.
+constexpr int kStaticMaxDevices = 64;
+static std::atomic<unsigned char*> g_sssp_scratch_ptr[kStaticMaxDevices];
+
+extern "C" uint32_t ts_sssp_static_max_nodes(void) { return kStaticMaxNodes; }
+
+extern "C" int ts_sssp_static(uint32_t n_nodes, uint32_t n_edges, const uint32_t* d_out_off, const uint32_t* d_out_edge,
+                              const uint32_t* d_edge_to, const uint32_t* d_w, const uint32_t* d_sources,
+                              uint32_t n_sources, uint32_t* d_pred, uint32_t* d_error, void* cuda_stream) {
+    if (n_nodes == 0 || n_edges == 0) return fail(TS_EINVAL, "empty graph");
+    if (n_nodes > kStaticMaxNodes)
+        return fail(TS_EINVAL, "ts_sssp_static: %u nodes exceed the %u its static scratch of %zu MiB is sized for "
+                               "(use ts_reroute / ts_sue_solve with a caller-owned workspace)", n_nodes, kStaticMaxNodes,
+                    kStaticScratchBytes >> 20);
+    if (!d_out_off || !d_out_edge || !d_edge_to || !d_w || (n_sources && (!d_sources || !d_pred)))
+        return fail(TS_EINVAL, "null argument");
+    if (n_sources == 0) return TS_OK;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(TS_EINVAL, "device ordinal %d beyond %d", dev, kStaticMaxDevices);
+    unsigned char* scratch = g_sssp_scratch_ptr[dev].load(std::memory_order_acquire);
+    if (!scratch) {                                  // set-up, once per device, with that device current
+        void* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_sssp_scratch));
+        scratch = static_cast<unsigned char*>(p);
+        g_sssp_scratch_ptr[dev].store(scratch, std::memory_order_release);
+    }
+    const uint64_t per_tree = (uint64_t)n_nodes * kStaticBytesPerNode;
+    const uint32_t ctas = (uint32_t)std::min<uint64_t>({(uint64_t)kRrCtas, (uint64_t)n_sources, kStaticScratchBytes / per_tree});
+    k_sssp_static<<<ctas, kRrThreads, 0, (cudaStream_t)cuda_stream>>>(scratch, n_nodes, d_out_off, d_out_edge, d_edge_to, d_w,
+                                                                       d_sources, n_sources, d_pred, d_error);
+    CUDA_TRY(cudaGetLastError());
+    return TS_OK;
+}
