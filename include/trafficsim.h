@@ -306,6 +306,16 @@ typedef struct ts_sue_out {
 int ts_sue_workspace(const ts_sue_problem *problem, size_t *bytes);
 int ts_sue_solve(const ts_sue_problem *problem, const ts_device *dev, ts_sue_out *out);
 
+/* Checkpoint / resume.  The workspace is the caller's, so a checkpoint is a copy of it (the step kernels' whole
+ * state: slots, atlas, claims, queues, statistics, the route table in use) behind a small header with the
+ * host-side counters.  ts_checkpoint_size gives the bytes, ts_checkpoint fills a HOST buffer of that size,
+ * ts_restore puts a simulation created from the SAME inputs back into that state (checked: TS_EINVAL if the
+ * layout differs or the buffer is not a checkpoint); stepping on from there gives bit for bit what the
+ * uninterrupted run gives.  Tuning options (ts_set_option) are not part of it.  Both calls synchronise. */
+int ts_checkpoint_size(ts_sim *sim, size_t *bytes);
+int ts_checkpoint(ts_sim *sim, void *host_buf);
+int ts_restore(ts_sim *sim, const void *host_buf);
+
 /* Shortest-path trees WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph
  * capture, tight serving loops, harnesses that forbid it): the tree kernel of ts_reroute / ts_sue_solve
  * (readings R37-R38) with its scratch -- per tree in flight a 64-bit label, two frontier words and

@@ -17,7 +17,7 @@ TS_OK, TS_EINVAL, TS_ENOMEM, TS_ECUDA, TS_EINVARIANT = 0, -1, -2, -3, -4
 
 EXPORTS = ["ts_query_workspace", "ts_create", "ts_step", "ts_step_digest", "ts_reset",
            "ts_read_state", "ts_read_edge_stats", "ts_set_option", "ts_read_profile",
-           "ts_read_emissions", "ts_read_utilisation", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_sssp_static", "ts_sssp_static_max_nodes", "ts_destroy", "ts_last_error", "ts_version"]
+           "ts_read_emissions", "ts_read_utilisation", "ts_reroute", "ts_read_routes", "ts_sue_workspace", "ts_sue_solve", "ts_sssp_static", "ts_sssp_static_max_nodes", "ts_checkpoint_size", "ts_checkpoint", "ts_restore", "ts_destroy", "ts_last_error", "ts_version"]
 
 _u32p, _u8p, _f32p, _u64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint8), C.POINTER(C.c_float),
                              C.POINTER(C.c_uint64))
@@ -122,6 +122,11 @@ def load():
         L.ts_destroy.restype = None
         L.ts_last_error.restype = C.c_char_p
         L.ts_version.restype = C.c_char_p
+        L.ts_checkpoint_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ts_checkpoint.argtypes = [C.c_void_p, C.c_void_p]
+        L.ts_restore.argtypes = [C.c_void_p, C.c_void_p]
+        for n in ("ts_checkpoint_size", "ts_checkpoint", "ts_restore"):
+            getattr(L, n).restype = C.c_int
         L.ts_sssp_static.argtypes = [C.c_uint32, C.c_uint32] + [C.c_void_p] * 5 + [C.c_uint32] + [C.c_void_p] * 3
         L.ts_sssp_static.restype = C.c_int
         L.ts_sssp_static_max_nodes.restype = C.c_uint32
@@ -247,6 +252,19 @@ class Sim:
         edges = np.zeros(int(n.value), np.uint32)
         _check(load().ts_read_routes(self._h, off.ctypes.data, edges.ctypes.data, C.byref(n)))
         return off, edges
+
+    def checkpoint(self):
+        """ts_checkpoint: the whole state as one host byte array (numpy uint8)."""
+        n = C.c_size_t()
+        _check(load().ts_checkpoint_size(self._h, C.byref(n)))
+        buf = np.empty(n.value, np.uint8)
+        _check(load().ts_checkpoint(self._h, buf.ctypes.data))
+        return buf
+
+    def restore(self, buf):
+        """ts_restore: back to the state of a checkpoint of a simulation created from the same inputs."""
+        buf = np.ascontiguousarray(buf, np.uint8)
+        _check(load().ts_restore(self._h, buf.ctypes.data))
 
     def read_counts(self):
         """Scalars only (no per-vehicle arrays are copied)."""

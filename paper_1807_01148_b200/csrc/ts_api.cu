@@ -1564,3 +1564,51 @@ extern "C" int ts_sssp_static(uint32_t n_nodes, uint32_t n_edges, const uint32_t
     CUDA_TRY(cudaGetLastError());
     return TS_OK;
 }
+
+// ------------------------------------------------------------------ checkpoint / resume
+//
+// The caller owns the whole workspace, so a checkpoint is a copy of it (without the shortest-path scratch of
+// ts_reroute, which holds nothing between calls) behind a small header with the host-side counters.  Restoring
+// needs a simulation created from the SAME inputs (same layout); the header is checked for that.
+struct CheckpointHeader {
+    uint64_t magic, ws_bytes, total;
+    uint32_t V, E, N, k, cur, chunk_no, route_cur, n_queues, sticky, pad;
+};
+static constexpr uint64_t kCheckpointMagic = 0x31544B4350435354ull;   // "TSCPCKT1"
+
+static size_t checkpoint_ws_bytes(const ts_sim* s) { return s->L.Rcap ? s->L.rr_pred : s->L.total; }
+
+extern "C" int ts_checkpoint_size(ts_sim* s, size_t* bytes) {
+    if (!s || !bytes) return fail(TS_EINVAL, "null argument");
+    *bytes = sizeof(CheckpointHeader) + checkpoint_ws_bytes(s);
+    return TS_OK;
+}
+
+extern "C" int ts_checkpoint(ts_sim* s, void* host_buf) {
+    if (!s || !host_buf) return fail(TS_EINVAL, "null argument");
+    if (s->sticky) return fail(TS_EINVARIANT, "sticky device error 0x%x", s->sticky);
+    CheckpointHeader h;
+    memset(&h, 0, sizeof h);
+    h.magic = kCheckpointMagic; h.ws_bytes = checkpoint_ws_bytes(s); h.total = s->L.total;
+    h.V = s->L.V; h.E = s->L.E; h.N = s->L.N; h.k = s->k; h.cur = s->cur; h.chunk_no = s->chunk_no;
+    h.route_cur = s->route_cur; h.n_queues = s->ctx.n_queues; h.sticky = s->sticky;
+    memcpy(host_buf, &h, sizeof h);
+    CUDA_TRY(cudaMemcpyAsync((uint8_t*)host_buf + sizeof h, s->ws, h.ws_bytes, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return TS_OK;
+}
+
+extern "C" int ts_restore(ts_sim* s, const void* host_buf) {
+    if (!s || !host_buf) return fail(TS_EINVAL, "null argument");
+    CheckpointHeader h;
+    memcpy(&h, host_buf, sizeof h);
+    if (h.magic != kCheckpointMagic) return fail(TS_EINVAL, "not a checkpoint of this library");
+    if (h.total != s->L.total || h.ws_bytes != checkpoint_ws_bytes(s) || h.V != s->L.V || h.E != s->L.E || h.N != s->L.N)
+        return fail(TS_EINVAL, "the checkpoint was taken from a simulation with other inputs (workspace layout differs)");
+    CUDA_TRY(cudaMemcpyAsync(s->ws, (const uint8_t*)host_buf + sizeof h, h.ws_bytes, cudaMemcpyHostToDevice, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    s->k = h.k; s->cur = h.cur; s->chunk_no = h.chunk_no; s->sticky = h.sticky;
+    s->route_cur = h.route_cur; s->ctx.n_queues = h.n_queues;
+    if (s->L.Rcap) s->ctx.route_edges = at<uint32_t>(s, h.route_cur ? s->L.rr_routes2 : s->L.route_edges);
+    return TS_OK;
+}

@@ -212,3 +212,57 @@ def test_signal_plans_of_every_shape(seed):
         _compare(corridor(n_edges=2, length=300, departs=np.arange(8) * 3.0, ctrl=2, sig=one), 600, 1)
         two = (np.full(n, 1), np.full(n, 1), np.full(n, 7))            # cycle 2: green on alternate steps
         _compare(corridor(n_edges=2, length=300, departs=np.arange(8) * 3.0, ctrl=2, sig=two), 600, 1)
+
+
+def test_checkpoint_and_resume_give_the_uninterrupted_run():
+    """ts_checkpoint / ts_restore: stepping on from a restored checkpoint reproduces, digest by digest, what the
+    uninterrupted run (and the oracle) give -- across a re-sort boundary, in the adaptive launch scheme, into a
+    second simulation object created from the same inputs, and with a re-routed demand in the workspace."""
+    import paper_1807_01148_b200 as pkg
+    from oracle import Oracle
+    from paper_1807_01148_b200 import workload as W
+    b = small_signal_grid()
+    b = dict(b, params=dict(b["params"], emissions=1, route_capacity=2 * len(b["route_edges"]) + 1024))
+    want = Oracle(b).step(1500, digests=True)
+    sim = pkg.Sim(b, "cuda:0")
+    sim.set_option("adaptive_chunk", 64)
+    assert np.array_equal(sim.step_digest(700), want[:700])
+    snap = sim.checkpoint()
+    assert np.array_equal(sim.step_digest(800), want[700:])                  # the uninterrupted run
+    first = sim.read_state()
+    sim.restore(snap)
+    assert sim.read_counts()["step"] == 700
+    assert np.array_equal(sim.step_digest(800), want[700:])                  # resumed in place
+    again = sim.read_state()
+    for key in ("status", "edge", "lane", "route_idx", "insert_step", "arrive_step"):
+        assert np.array_equal(first[key], again[key]), key
+    assert np.array_equal(first["x"].view(np.uint32), again["x"].view(np.uint32))
+    ea, eb = sim.read_emissions(), None
+    other = pkg.Sim(b, "cuda:0")                                             # a fresh object, same inputs
+    other.restore(snap)
+    assert np.array_equal(other.step_digest(800), want[700:])
+    eb = other.read_emissions()
+    assert np.array_equal(ea["fuel_ml"].view(np.uint32), eb["fuel_ml"].view(np.uint32))
+    es1, es2 = sim.read_edge_stats(), other.read_edge_stats()
+    for key in es1:
+        assert np.array_equal(es1[key], es2[key]), key
+    # a checkpoint taken after ts_reroute carries the new routes and queues
+    wf = W.free_flow_weights(b)
+    other.reroute(wf, W.reroute_mask(b["n_vehicles"], 2))
+    off, edges = other.read_routes()
+    snap2 = other.checkpoint()
+    d1 = other.step_digest(600)
+    other.reroute(wf)                                                        # something else in the workspace
+    other.restore(snap2)
+    o2, e2 = other.read_routes()
+    assert np.array_equal(off, o2) and np.array_equal(edges, e2)
+    assert np.array_equal(other.step_digest(600), d1)
+    assert np.array_equal(d1, Oracle(dict(b, route_off=off, route_edges=edges)).step(600, digests=True))
+    # refused: a checkpoint of other inputs, or no checkpoint at all
+    small = pkg.Sim(W.config1(), "cuda:0")
+    with pytest.raises(pkg.TsError):
+        small.restore(snap)
+    with pytest.raises(pkg.TsError):
+        sim.restore(np.zeros(len(snap), np.uint8))
+    for s_ in (sim, other, small):
+        s_.close()
