@@ -267,9 +267,19 @@ __device__ __forceinline__ Who who() {
 }
 
 // Grid-wide barrier of the persistent kernel: one arrival per CTA on a monotonic counter.
-// bar.sync orders the CTA's writes before thread 0's release; the acquire load plus the second
-// bar.sync orders them before every later read of any thread (mutable data is read with ld.cg,
-// i.e. from L2, so no stale L1 line can be observed).
+// bar.sync orders the CTA's writes before thread 0's release (red.release.gpu: cumulative, one
+// MEMBAR.ALL.GPU); thread 0 polls the counter with relaxed loads and the second bar.sync hands the
+// observation on to the CTA.
+//
+// There is deliberately NO gpu-scope fence on the acquiring side.  What such a fence adds in hardware is
+// CCTL.IVALL, the invalidation of the SM's whole L1 -- needed by readers that use L1-cached loads of data
+// other SMs write.  This kernel has none: everything any thread writes during a launch (slot state, atlas,
+// claims, queues, counters, sort scratch) is read with ld.global.cg / atomics, i.e. at L2, the point of
+// coherence (LDG.E.STRONG.GPU in the SASS; the only other loads are ld.global.nc of data no thread writes
+// during a launch: edge records, routes, queue and departure records).  A load issued after the poll has
+// returned reaches L2 after the releasing CTA's writes were performed there.  Keeping L1 alive across the
+// 2 barriers of every step is what lets the edge records of a CTA's vehicles be L1 hits step after step
+// (`__threadfence()` = MEMBAR.SC.GPU + CCTL.IVALL dropped them four times per step).
 struct PhaseClock;
 __device__ __forceinline__ void clock_tick(PhaseClock& clk, int b);
 
@@ -279,13 +289,11 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
     __syncthreads();
     if (threadIdx.x == 0) {
         clock_tick(clk, b);
-        __threadfence();                                          // release, cumulative over the CTA
-        asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
         unsigned int v;
-        do {                                                      // poll without a fence per probe
+        do {
             asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(counter) : "memory");
         } while ((int)(v - target) < 0);
-        __threadfence();                                          // acquire
     }
     __syncthreads();
 }
@@ -383,7 +391,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_persistent(const __grid_constant__ 
     if (clk.acc) {                                  // mean over CTAs per bin; slowest CTA's phase 1
         for (int b = 0; b < 6; b++) atomicAdd(&c.dyn->prof[b], sh_prof[b] / me.n_cta);
         atomicMax(&c.dyn->prof[7], sh_prof[0]);
-        if (me.cta == 0) c.dyn->prof[6] += n;
+        if (me.cta == 0) c.dyn->prof[6] = __ldcg(&c.dyn->prof[6]) + n;
     }
     // more warps pay once a CTA has more than one round of tiles at the small size
     if (variant != 2u && me.cta == 0 && me.t == 0)

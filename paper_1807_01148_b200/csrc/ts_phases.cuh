@@ -443,7 +443,7 @@ __device__ __forceinline__ void phase2(const Ctx& c, const Slots& S, uint32_t k,
         // every slot handed out in phase 1 takes part from the next step on
         c.dyn->n_slots = min(__ldcg(&c.dyn->slot_alloc), c.cap_slots);
         c.dyn->k = k + 1;
-        if (sample) c.dyn->n_samples += 1;
+        if (sample) c.dyn->n_samples = __ldcg(&c.dyn->n_samples) + 1;
     }
     for (uint32_t j = 0;; j++) {
         const uint32_t s = me.slot(j);
