@@ -354,6 +354,8 @@ def main():
     ap.add_argument("--threads", type=int, default=0, help="CTA size of the persistent kernel (tuning)")
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     ap.add_argument("--sort-period", type=int, default=-1, help="steps between compaction + re-sort (tuning)")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="ts_set_option(KEY, VALUE) before the run (tuning knobs; results never depend on them)")
     ap.add_argument("--profile", action="store_true", help="clock the phases inside the persistent kernel")
     ap.add_argument("--emissions", action="store_true",
                     help="keep the per-vehicle CO / fuel totals of PAPER.md:408-423 (SURVEY.md 8(f) row 2) during the run")
@@ -410,6 +412,9 @@ def main():
         tuning["sort_period"] = args.sort_period
     if args.profile:
         tuning["profile"] = 1
+    for kv in args.opt:
+        key, _, val = kv.partition("=")
+        tuning[key] = int(val)
     for key, val in tuning.items():
         sim.set_option(key, val)
 

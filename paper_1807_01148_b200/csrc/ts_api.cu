@@ -240,6 +240,11 @@ struct ts_sim {
     int blocks_per_sm = 1;
     uint32_t chunk_no = 0;    // adaptive chunks enqueued since ts_reset (parity selects Dyn::prefer_big[])
     uint32_t adaptive_chunk = 2048;   // steps per adaptive chunk
+    // Most move-record tiles per thread kept in shared memory.  Shared memory and L1 are one 228 KB array: what the
+    // move records do not take stays L1, which holds the edge records of the SM's vehicles across steps (the grid
+    // barrier keeps L1 alive).  Records beyond the limit go through L2 (Ctx::mr_g).  Measured: config 4 (3 M slots:
+    // the records would take all of it) 11.2 -> 14.1 G vehicle-updates/s, config 3 17.7 -> 18.0, config 5 3.72 -> 3.88.
+    uint32_t smem_tiles = 6;
     long long adaptive_above = -1;    // live slots above which the big CTA size is preferred (-1: one round of tiles at 640 threads)
     int adaptive = 1;         // no CTA size asked for: 640 threads, or 896 while more than one round of tiles is live
     int sms = 0;
@@ -915,6 +920,9 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
     } else if (!strcmp(key, "adaptive_chunk")) {
         if (value < 1 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "adaptive_chunk must be >= 1");
         s->adaptive_chunk = (uint32_t)value;
+    } else if (!strcmp(key, "smem_tiles")) {
+        if (value < 0 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "smem_tiles must be >= 0");
+        s->smem_tiles = (uint32_t)value;
     } else if (!strcmp(key, "adaptive_above")) {
         if (value < -1 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "adaptive_above must be >= -1");
         s->adaptive_above = value;
@@ -952,7 +960,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             const uint32_t grid = (uint32_t)(s->sms * s->blocks_per_sm);
             if (grid > kMaxCtas) return fail(TS_EINVAL, "step kernel: %u CTAs exceed the %u the sort scratch is sized for", grid, kMaxCtas);
             const uint32_t need_j = (s->L.cap + grid * threads - 1) / (grid * threads);
-            mr_j = std::min(mr_j, need_j);
+            mr_j = std::min(std::min(mr_j, need_j), s->smem_tiles);
             const size_t smem = (size_t)mr_j * 16 * threads;
             const void* kern = step_kernel(threads * s->blocks_per_sm, s->L.emissions != 0, s->L.ext != 0);
             int per_sm = 0;
