@@ -353,6 +353,9 @@ int ts_sssp_static(uint32_t n_nodes, uint32_t n_edges, const uint32_t *d_out_off
  *  "sort_period"   steps between compaction of retired slots + re-sort of the live ones by
  *                  edge; 0 = never; default 128 (256 on networks
  *                  with more than 4 M sort keys).
+ *  "sort_groups"   the re-sort key is (vehicle id & (sort_groups - 1), edge): a power of two between 1 (by edge
+ *                  alone) and the lane-change period when that is a power of two <= 8 (the default: whole
+ *                  warps then take or skip the lane-change code together).
  *  "smem_tiles"    most tiles (one vehicle per thread) whose move records the persistent kernel keeps in
  *                  shared memory; the rest go through L2.  Shared memory and L1 share one array per
  *                  SM: what the records leave stays L1 for the edge records.  Default 6.

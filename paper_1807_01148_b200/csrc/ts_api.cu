@@ -920,6 +920,10 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
     } else if (!strcmp(key, "adaptive_chunk")) {
         if (value < 1 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "adaptive_chunk must be >= 1");
         s->adaptive_chunk = (uint32_t)value;
+    } else if (!strcmp(key, "sort_groups")) {
+        if (value < 1 || value > (long long)s->L.groups || (value & (value - 1)))
+            return fail(TS_EINVAL, "sort_groups must be a power of two in 1..%u (the lane-change period of this simulation)", s->L.groups);
+        s->ctx.sort_groups = (uint32_t)value;
     } else if (!strcmp(key, "smem_tiles")) {
         if (value < 0 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "smem_tiles must be >= 0");
         s->smem_tiles = (uint32_t)value;

@@ -68,6 +68,9 @@ def test_mixed_controls(mode):
     dict(adaptive_chunk=37, adaptive_above=0),     # adaptive CTA size: 896 threads from the second chunk on
     dict(adaptive_chunk=50, adaptive_above=700),   # ... switching both ways as the slot count crosses 700
     dict(adaptive_chunk=1, adaptive_above=300, sort_period=5),
+    dict(smem_tiles=0, threads=64, sort_period=16),    # every move record through L2
+    dict(smem_tiles=1, threads=96, sort_groups=1),     # one tile in shared memory; re-sort by edge alone
+    dict(sort_groups=2, sort_period=9),
 ])
 def test_results_do_not_depend_on_slot_order(options):
     """A9/A10: compaction and the edge re-sort change where a vehicle's state lives, never what
