@@ -185,7 +185,10 @@ int ts_query_workspace(const ts_network *net, const ts_routes *routes,
  * library copies what it needs and keeps none.  *out is NULL on failure.
  * Errors: TS_EINVAL (sizes, ranges, a route that is not contiguous, look-ahead or entry zone shorter
  * than one step's advance, signal cycle beyond 2^24 steps, ...), TS_ENOMEM (workspace smaller than
- * ts_query_workspace says), TS_ECUDA (no device: there is no CPU fallback). */
+ * ts_query_workspace says), TS_ECUDA (no device: there is no CPU fallback).
+ * The host work (validation, departure-queue index) runs on up to 16 threads; the copy of the route table, the
+ * largest input, is enqueued first and overlaps it when the caller's buffer is pinned.  With the environment
+ * variable TS_TRACE_CREATE set, the milliseconds of each stage go to stderr. */
 int ts_create(const ts_network *net, const ts_routes *routes, const ts_departures *dep,
               const ts_params *params, const ts_device *dev, ts_sim **out);
 

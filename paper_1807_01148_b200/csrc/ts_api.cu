@@ -6,6 +6,8 @@
 // (mode 1, default): the step is bound by the two grid-wide dependencies, not by bandwidth,
 // so no host launch may sit inside the loop.
 #include <cooperative_groups.h>
+#include <chrono>
+#include <memory>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -546,36 +548,80 @@ static const void* step_kernel(int per_sm_threads, bool emissions, bool ext) {
 // departure record per vehicle in queue order { id, v0_mult, mand, route begin } { route end, second
 // edge, departure step, type } and one 16-byte record per queue { row of lane 0, lane_base, end, edge }.
 // Used by ts_create and, for the new first edges, by ts_reroute.
+// A host array that is NOT zero-filled when it is made: its pages are first touched by the threads that fill it.
+struct DepRecBuf {
+    std::unique_ptr<uint4[]> p;
+    void alloc(size_t n) { p.reset(new uint4[n]); }
+    uint4* data() { return p.get(); }
+    uint4& operator[](size_t i) { return p[i]; }
+};
+
 static void build_queues(uint32_t V, uint32_t E, const std::vector<EdgeRec>& edges, const uint32_t* first,
                          const uint32_t* second, const uint32_t* rbegin, const uint32_t* rend,
                          const uint32_t* dep_step, const uint32_t* v0m_bits, const uint32_t* mand_bits,
-                         const uint32_t* type, std::vector<uint4>& dep_rec, std::vector<uint4>& queue_rec) {
+                         const uint32_t* type, DepRecBuf& dep_rec, std::vector<uint4>& queue_rec) {
     // counting sort by first edge (ids stay ascending inside an edge), then each queue by
     // departure step, stable -- i.e. by (edge, departure step, id) -- queues in parallel
+    const bool trace = getenv("TS_TRACE_CREATE") != nullptr;
+    auto t_last = std::chrono::steady_clock::now();
+    auto lap = [&](const char* what) {
+        if (!trace) return;
+        const auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "  build_queues: %-24s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(t - t_last).count());
+        t_last = t;
+    };
     std::vector<uint32_t> order(V), q_begin((size_t)E + 1, 0);
-    for (uint32_t i = 0; i < V; i++) q_begin[first[i] + 1]++;
-    for (uint32_t e = 0; e < E; e++) q_begin[e + 1] += q_begin[e];
     {
-        std::vector<uint32_t> fill(q_begin.begin(), q_begin.end() - 1);
-        for (uint32_t i = 0; i < V; i++) order[fill[first[i]]++] = i;
+        // T contiguous blocks of vehicles, one histogram each; block t's vehicles of edge e go behind those of
+        // blocks 0..t-1: ids stay ascending inside an edge
+        const size_t T = std::max<size_t>(1, std::min<size_t>({(size_t)16, (size_t)V / 65536 + 1, ((size_t)1 << 20) / ((size_t)E + 1) + 1,
+                                                             (size_t)std::max(1u, std::thread::hardware_concurrency())}));
+        const size_t per = ((size_t)V + T - 1) / T;
+        std::vector<uint32_t> hist(T * (size_t)E, 0);
+        auto blocks = [&](auto fn) {
+            if (T == 1) { fn((size_t)0); return; }
+            std::vector<std::thread> th;
+            for (size_t t = 0; t < T; t++) th.emplace_back([=] { fn(t); });
+            for (auto& x : th) x.join();
+        };
+        blocks([&](size_t t) {
+            uint32_t* h = hist.data() + t * (size_t)E;
+            for (size_t i = std::min((size_t)V, t * per), e_ = std::min((size_t)V, i + per); i < e_; i++) h[first[i]]++;
+        });
+        uint32_t run = 0;
+        for (uint32_t e = 0; e < E; e++) {
+            q_begin[e] = run;
+            for (size_t t = 0; t < T; t++) { const uint32_t c = hist[t * (size_t)E + e]; hist[t * (size_t)E + e] = run; run += c; }
+        }
+        q_begin[E] = run;
+        blocks([&](size_t t) {
+            uint32_t* h = hist.data() + t * (size_t)E;
+            for (size_t i = std::min((size_t)V, t * per), e_ = std::min((size_t)V, i + per); i < e_; i++) order[h[first[i]]++] = (uint32_t)i;
+        });
     }
+    lap("counting sort");
     parallel_chunks(E, [&](size_t b, size_t e_, size_t) {
         for (size_t e = b; e < e_; e++)
             if (q_begin[e + 1] - q_begin[e] > 1)
-                std::stable_sort(order.begin() + q_begin[e], order.begin() + q_begin[e + 1],
-                                 [&](uint32_t x, uint32_t y) { return dep_step[x] < dep_step[y]; });
+                std::sort(order.begin() + q_begin[e], order.begin() + q_begin[e + 1],     // ids were ascending: (step, id) is the stable order
+                          [&](uint32_t x, uint32_t y) { return dep_step[x] != dep_step[y] ? dep_step[x] < dep_step[y] : x < y; });
     });
-    dep_rec.assign(2 * (size_t)V, make_uint4(0, 0, 0, 0));
+    lap("sort inside queues");
+    // one queue per first edge that has vehicles, in edge order; its records are the next q_begin[e+1] - q_begin[e]
     queue_rec.clear();
-    for (uint32_t n = 0; n < V; n++) {
-        const uint32_t i = order[n], e = first[i];
-        if (n == 0 || e != queue_rec.back().w) {
-            if (!queue_rec.empty()) queue_rec.back().z = n;
-            queue_rec.push_back(make_uint4(edges[e].row, edges[e].lane_base, V, e));
+    for (uint32_t e = 0; e < E; e++)
+        if (q_begin[e + 1] > q_begin[e])
+            queue_rec.push_back(make_uint4(edges[e].row, edges[e].lane_base, q_begin[e + 1], e));
+    lap("queue records");
+    dep_rec.alloc(2 * (size_t)V);
+    parallel_chunks(V, [&](size_t b, size_t e_, size_t) {
+        for (size_t n = b; n < e_; n++) {
+            const uint32_t i = order[n];
+            dep_rec[2 * n] = make_uint4(i, v0m_bits[i], mand_bits[i], rbegin[i]);
+            dep_rec[2 * n + 1] = make_uint4(rend[i], second[i], dep_step[i], type[i]);
         }
-        dep_rec[2 * (size_t)n] = make_uint4(i, v0m_bits[i], mand_bits[i], rbegin[i]);
-        dep_rec[2 * (size_t)n + 1] = make_uint4(rend[i], second[i], dep_step[i], type[i]);
-    }
+    });
+    lap("dep_rec fill");
 }
 
 static int validate(const ts_network* net, const ts_routes* rt, const ts_departures* dep, const ts_params* p) {
@@ -597,18 +643,41 @@ static int validate(const ts_network* net, const ts_routes* rt, const ts_departu
             return fail(TS_EINVAL, "params: vehicle type %u needs type_len >= 2, type_a > 0, type_vmax > 0", t);
         max_len = std::max(max_len, p->type_len[t]); max_a = std::max(max_a, p->type_a[t]);
     }
-    if (dep->veh_type)
-        for (uint32_t i = 0; i < V; i++)
-            if (dep->veh_type[i] >= std::max(1u, p->n_types)) return fail(TS_EINVAL, "vehicle %u: veh_type %u out of range", i, dep->veh_type[i]);
+    // per vehicle, in parallel: the first offending vehicle (lowest id) is the one reported
     float max_mult = 1.0f;
-    for (uint32_t i = 0; i < V; i++) {
-        if (dep->v0_mult) {
-            if (!(dep->v0_mult[i] > 0)) return fail(TS_EINVAL, "vehicle %u: v0_mult must be > 0", i);
-            max_mult = std::max(max_mult, dep->v0_mult[i]);
+    {
+        std::atomic<uint32_t> bad(0xFFFFFFFFu);
+        std::vector<float> chunk_max(64, 1.0f);
+        const uint32_t n_types = std::max(1u, p->n_types);
+        auto note = [&](uint32_t i) {
+            uint32_t cur = bad.load();
+            while (i < cur && !bad.compare_exchange_weak(cur, i)) {}
+        };
+        auto wrong = [&](uint32_t i) -> int {          // 0 = fine, else which rule it breaks
+            if (dep->veh_type && dep->veh_type[i] >= n_types) return 1;
+            if (dep->v0_mult && !(dep->v0_mult[i] > 0)) return 2;
+            if (!(dep->depart_time_s[i] >= 0)) return 3;
+            if (std::ceil((double)dep->depart_time_s[i] / (double)p->dt) >= 2147483648.0) return 4;
+            return 0;
+        };
+        parallel_chunks(V, [&](size_t b, size_t e_, size_t t) {
+            float m = 1.0f;
+            for (size_t i = b; i < e_; i++) {
+                if (wrong((uint32_t)i)) { note((uint32_t)i); break; }
+                if (dep->v0_mult) m = std::max(m, dep->v0_mult[i]);
+            }
+            chunk_max[t] = m;
+        });
+        const uint32_t i = bad.load();
+        if (i != 0xFFFFFFFFu) {
+            switch (wrong(i)) {
+                case 1: return fail(TS_EINVAL, "vehicle %u: veh_type %u out of range", i, dep->veh_type[i]);
+                case 2: return fail(TS_EINVAL, "vehicle %u: v0_mult must be > 0", i);
+                case 3: return fail(TS_EINVAL, "vehicle %u: negative departure time", i);
+                default: return fail(TS_EINVAL, "vehicle %u: departure step beyond 2^31", i);
+            }
         }
-        if (!(dep->depart_time_s[i] >= 0)) return fail(TS_EINVAL, "vehicle %u: negative departure time", i);
-        if (std::ceil((double)dep->depart_time_s[i] / (double)p->dt) >= 2147483648.0)
-            return fail(TS_EINVAL, "vehicle %u: departure step beyond 2^31", i);
+        for (float m : chunk_max) max_mult = std::max(max_mult, m);
     }
     float max_vlim = 0.0f;
     for (uint32_t e = 0; e < E; e++) {
@@ -744,14 +813,33 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(TS_ECUDA, "no CUDA device: this library has no CPU fallback");
+    const bool trace = getenv("TS_TRACE_CREATE") != nullptr;
+    auto t_last = std::chrono::steady_clock::now();
+    auto lap = [&](const char* what) {
+        if (!trace) return;
+        const auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "ts_create: %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(t - t_last).count());
+        t_last = t;
+    };
     Layout L;
     std::vector<uint32_t> first_edge;
     int rc = plan_sizes(net, rt, p, L, &first_edge);
+    lap("plan_sizes");
     if (rc) return rc;
     if ((uint64_t)L.groups * L.E >= 0xFFFFFFF0ull) L.groups = 1;
-    if ((rc = validate(net, rt, dep, p))) return rc;
     if (!dev->workspace || ((uintptr_t)dev->workspace & 255)) return fail(TS_EINVAL, "workspace must be a 256-byte aligned device pointer");
     if (dev->bytes < L.total) return fail(TS_ENOMEM, "workspace too small: %zu < %zu bytes", dev->bytes, L.total);
+    if (!net || !rt || !rt->route_edges) return fail(TS_EINVAL, "null argument");
+    // the routes are by far the largest input (4 bytes per route entry): their copy is enqueued first and travels
+    // while the host validates and builds its records (from pinned memory; a pageable buffer is staged at once)
+    const cudaError_t ce_routes = L.R ? cudaMemcpyAsync((uint8_t*)dev->workspace + L.route_edges, rt->route_edges, L.R * 4,
+                                                        cudaMemcpyHostToDevice, (cudaStream_t)dev->cuda_stream) : cudaSuccess;
+    if (ce_routes != cudaSuccess) return fail(TS_ECUDA, "upload: %s", cudaGetErrorString(ce_routes));
+    if ((rc = validate(net, rt, dep, p))) {
+        cudaStreamSynchronize((cudaStream_t)dev->cuda_stream);      // the caller may free its buffers on an error
+        return rc;
+    }
+    lap("validate");
 
     const uint32_t V = L.V, E = L.E, N = L.N;
     // per-edge records: atlas row offsets, claim indices, signal plan of the head node
@@ -797,28 +885,32 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         r.off_sh = (uint32_t)off | (sh1 << 24) | (sh2 << 25);
         r.green = (uint16_t)net->sig_green_steps[h];
     }
+    lap("edge records");
     // departure queues: per first edge, FIFO by (departure step, id) (R19)
     std::vector<uint32_t> dep_step(V), route_begin(V);
-    for (uint32_t i = 0; i < V; i++) {
-        dep_step[i] = (uint32_t)std::ceil((double)dep->depart_time_s[i] / (double)p->dt);
-        route_begin[i] = (uint32_t)rt->route_off[i];
-    }
     const uint32_t* re = rt->route_edges;
     auto fbits = [](float f) { uint32_t u; memcpy(&u, &f, 4); return u; };
     std::vector<uint32_t> second(V), route_end(V), v0m_bits(V), mand_bits(V), type_v(V);
-    for (uint32_t i = 0; i < V; i++) {
-        const uint32_t rb = route_begin[i], rend = (uint32_t)rt->route_off[i + 1];
-        route_end[i] = rend;
-        second[i] = rb + 1 < rend ? re[rb + 1] : NONE32;
-        v0m_bits[i] = fbits(dep->v0_mult ? dep->v0_mult[i] : 1.0f);
-        mand_bits[i] = fbits(dep->mand_dist_m ? dep->mand_dist_m[i] : p->mand_dist_default);
-        type_v[i] = dep->veh_type ? dep->veh_type[i] : 0u;
-    }
-    std::vector<uint4> dep_rec, queue_rec;
+    parallel_chunks(V, [&](size_t b, size_t e_, size_t) {
+        for (size_t i = b; i < e_; i++) {
+            dep_step[i] = (uint32_t)std::ceil((double)dep->depart_time_s[i] / (double)p->dt);
+            const uint32_t rb = (uint32_t)rt->route_off[i], rend = (uint32_t)rt->route_off[i + 1];
+            route_begin[i] = rb;
+            route_end[i] = rend;
+            second[i] = rb + 1 < rend ? re[rb + 1] : NONE32;
+            v0m_bits[i] = fbits(dep->v0_mult ? dep->v0_mult[i] : 1.0f);
+            mand_bits[i] = fbits(dep->mand_dist_m ? dep->mand_dist_m[i] : p->mand_dist_default);
+            type_v[i] = dep->veh_type ? dep->veh_type[i] : 0u;
+        }
+    });
+    lap("per-vehicle arrays");
+    DepRecBuf dep_rec;
+    std::vector<uint4> queue_rec;
     build_queues(V, E, edges, first_edge.data(), second.data(), route_begin.data(), route_end.data(), dep_step.data(),
                  v0m_bits.data(), mand_bits.data(), type_v.data(), dep_rec, queue_rec);
     if (queue_rec.size() != L.Q) return fail(TS_EINVAL, "internal: queue count mismatch");
 
+    lap("build_queues");
     ts_sim* s = new ts_sim();
     s->L = L; s->ws = (uint8_t*)dev->workspace; s->stream = (cudaStream_t)dev->cuda_stream;
     s->out_on_device = dev->out_on_device;
@@ -830,7 +922,6 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     cudaError_t ce = cudaSuccess;
     auto chk = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
     chk(up(L.edges, edges.data(), (size_t)E * sizeof(EdgeRec)));
-    chk(up(L.route_edges, re, L.R * 4));
     chk(up(L.route_begin, route_begin.data(), (size_t)V * 4));
     chk(up(L.queue_rec, queue_rec.data(), (size_t)L.Q * 16));
     chk(up(L.dep_rec, dep_rec.data(), (size_t)V * 32));
@@ -882,8 +973,10 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         r.stamp = at<uint32_t>(s, L.rr_stamp); r.error = at<uint32_t>(s, L.rr_err);
     }
     // the staging vectors die with this scope: make sure the copies have left them
+    lap("enqueue copies, host copies");
     chk(cudaStreamSynchronize(st));
     if (ce != cudaSuccess) { delete s; return fail(TS_ECUDA, "upload: %s", cudaGetErrorString(ce)); }
+    lap("copies done");
 
     int dev_id = 0;
     cudaGetDevice(&dev_id);
@@ -902,6 +995,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
     // 36.5 / 33.3 / 33.2 / 33.4 on config 4 (10 M keys))
     s->sort_period = ((uint64_t)L.groups * L.E > 4000000ull) ? 256 : 128;
     if ((rc = ts_reset(s))) { delete s; return rc; }
+    lap("attributes, ts_reset enqueued");
     *out = s;
     return TS_OK;
 }
@@ -1274,7 +1368,8 @@ extern "C" int ts_reroute(ts_sim* s, const uint32_t* w_free, const uint8_t* mask
     CUDA_TRY(cudaMemcpyAsync(first2.data(), r.first2, (size_t)V * 8, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     for (uint32_t i = 0; i < V; i++) { first[i] = first2[2 * (size_t)i]; second[i] = first2[2 * (size_t)i + 1]; rend[i] = new_off[i] + new_len[i]; }
-    std::vector<uint4> dep_rec, queue_rec;
+    DepRecBuf dep_rec;
+    std::vector<uint4> queue_rec;
     build_queues(V, E, s->edges_h, first.data(), second.data(), new_off.data(), rend.data(), s->dep_step_h.data(),
                  s->v0m_bits_h.data(), s->mand_bits_h.data(), s->type_h.data(), dep_rec, queue_rec);
     if (queue_rec.size() > std::max(L.Q, L.Qcap)) return fail(TS_ENOMEM, "re-routing: %zu departure queues, room for %u", queue_rec.size(), std::max(L.Q, L.Qcap));
