@@ -1065,12 +1065,8 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
             if (per_sm < s->blocks_per_sm) return fail(TS_ECUDA, "step kernel: %d CTAs of %d threads do not fit on an SM", s->blocks_per_sm, threads);
             CUDA_TRY(cudaMemsetAsync(s->ctx.barrier, 0, 4, st));
-            // More warps pay once a CTA has more than one round of tiles at the small size -- as long
-            // as the atlas is L2-resident.  Where its gathers miss L2 (config 4: 460 MB) more warps
-            // measured slower (8.95 against 10.06 G vehicle-updates/s), so the small size stays.
-            const bool atlas_in_l2 = s->L.atlas_chunks * 144ull <= (unsigned long long)s->l2_bytes;
-            uint32_t big_above = s->adaptive_above >= 0 ? (uint32_t)s->adaptive_above
-                                 : atlas_in_l2 ? (uint32_t)s->sms * 640u : 0xFFFFFFFFu;
+            // More warps pay once a CTA has more than one round of tiles at the small size.
+            uint32_t big_above = s->adaptive_above >= 0 ? (uint32_t)s->adaptive_above : (uint32_t)s->sms * 640u;
             void* args[] = {&s->ctx, &k0, &m, &cur, (void*)&R, &mr_j, &dig, &s->profile, &variant, &big_above, &parity};
             CUDA_TRY(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, st));
             return TS_OK;
@@ -1085,6 +1081,11 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             // threads, more warps, best once CTAs hold several rounds of tiles); the device runs the
             // one the previous chunk asked for (Dyn::prefer_big) and the other returns at once.
             // Results do not depend on the launch geometry.
+            // The big size: 896 threads (28 warps, 72 registers) while the atlas is L2-resident; where its gathers
+            // miss L2 (config 4: 460 MB) the spills of that size cost more than its warps bring and 768 threads
+            // (24 warps, 85 registers) measured best: 14.43 against 14.13 (640) and 14.01 (896) G vehicle-updates/s.
+            const bool atlas_in_l2 = s->L.atlas_chunks * 144ull <= (unsigned long long)s->l2_bytes;
+            const int big_threads = atlas_in_l2 ? 896 : 768;
             const uint32_t chunk = s->adaptive_chunk;
             uint32_t k = s->k, cur = s->cur;
             for (uint32_t done = 0; done < n;) {
@@ -1092,7 +1093,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
                 unsigned long long* dig = d_digests ? d_digests + done : nullptr;
                 const uint32_t parity = s->chunk_no++ & 1u;
                 int rc = launch(k, m, cur, 640, 0u, dig, parity);
-                if (!rc) rc = launch(k, m, cur, 896, 1u, dig, parity);
+                if (!rc) rc = launch(k, m, cur, big_threads, 1u, dig, parity);
                 if (rc) {
                     // a chunk may have run on the device without the host's step counter following:
                     // the state is no longer usable until ts_reset
