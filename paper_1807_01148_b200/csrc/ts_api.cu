@@ -242,6 +242,7 @@ struct ts_sim {
     int blocks_per_sm = 1;
     uint32_t chunk_no = 0;    // adaptive chunks enqueued since ts_reset (parity selects Dyn::prefer_big[])
     uint32_t adaptive_chunk = 2048;   // steps per adaptive chunk
+    int adaptive_big = 0;             // CTA size of the big launch of a chunk; 0 = 896, or 768 where the atlas exceeds L2
     // Most move-record tiles per thread kept in shared memory.  Shared memory and L1 are one 228 KB array: what the
     // move records do not take stays L1, which holds the edge records of the SM's vehicles across steps (the grid
     // barrier keeps L1 alive).  Records beyond the limit go through L2 (Ctx::mr_g).  Measured: config 4 (3 M slots:
@@ -1014,6 +1015,9 @@ extern "C" int ts_set_option(ts_sim* s, const char* key, long long value) {
     } else if (!strcmp(key, "adaptive_chunk")) {
         if (value < 1 || value > 0x7FFFFFFF) return fail(TS_EINVAL, "adaptive_chunk must be >= 1");
         s->adaptive_chunk = (uint32_t)value;
+    } else if (!strcmp(key, "adaptive_big")) {
+        if (value != 0 && (value <= 640 || value > 1024 || value % 32)) return fail(TS_EINVAL, "adaptive_big must be 0 or a multiple of 32 in 672..1024");
+        s->adaptive_big = (int)value;
     } else if (!strcmp(key, "sort_groups")) {
         if (value < 1 || value > (long long)s->L.groups || (value & (value - 1)))
             return fail(TS_EINVAL, "sort_groups must be a power of two in 1..%u (the lane-change period of this simulation)", s->L.groups);
@@ -1085,7 +1089,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             // miss L2 (config 4: 460 MB) the spills of that size cost more than its warps bring and 768 threads
             // (24 warps, 85 registers) measured best: 14.43 against 14.13 (640) and 14.01 (896) G vehicle-updates/s.
             const bool atlas_in_l2 = s->L.atlas_chunks * 144ull <= (unsigned long long)s->l2_bytes;
-            const int big_threads = atlas_in_l2 ? 896 : 768;
+            const int big_threads = s->adaptive_big ? s->adaptive_big : atlas_in_l2 ? 896 : 768;
             const uint32_t chunk = s->adaptive_chunk;
             uint32_t k = s->k, cur = s->cur;
             for (uint32_t done = 0; done < n;) {
