@@ -14,6 +14,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <atomic>
@@ -83,6 +84,7 @@ struct Layout {
     uint32_t emissions = 0;
     uint32_t ext = 0;          // extended rule set: vehicle types and / or control variants (R31-R36)
     uint32_t typed = 0;        // more than one vehicle type: the atlas has a type plane
+    uint32_t cg = 0;           // code / type plane: one byte per 2^cg cells (Params::cg)
     // re-routing (ts_params.route_capacity != 0): a second route table, the graph in CSR form, one
     // shortest-path tree per distinct origin node, per-vehicle origin / destination / new offsets
     uint64_t Rcap = 0;         // entries per route table
@@ -103,7 +105,7 @@ struct Layout {
         route_begin = take((size_t)V * 4);
         queue_rec = take((size_t)Q * 16);
         dep_rec = take((size_t)V * 32);
-        codes = take(atlas_chunks * 128);
+        codes = take((atlas_chunks * 128) >> cg);
         occ = take((atlas_chunks + 3) * 16);          // one spare chunk in front, two behind: load_win never clamps
         queue_state = take((size_t)Q * 16); queue_cand = take((size_t)Q * 16);
         lane_claim = take(n_lanes * 8); node_claim = take((size_t)N * 8);
@@ -123,7 +125,7 @@ struct Layout {
         st_samp_code = take((size_t)E * 8);
         emis = take(emissions ? (size_t)V * 8 : 0);      // zeroed by ts_reset with the statistics
         digest = take((size_t)kDigestChunk * 8);
-        types = take(typed ? atlas_chunks * 128 : 0);
+        types = take(typed ? (atlas_chunks * 128) >> cg : 0);
         edge_aux = take(ext ? (size_t)E * 4 : 0); edge_from = take(ext ? (size_t)E * 4 : 0);
         node_free_from = take(ext ? (size_t)N * 4 : 0);
         if (Rcap) {
@@ -140,6 +142,19 @@ struct Layout {
         }
     }
 };
+
+// The code plane's granule (Params::cg).  A follower's advance is capped at the gap to its leader's cell
+// minus the leader's length (E2, E3), a lane change needs that gap on both sides (G1, G2) and an entrant
+// needs `insert_clear` free cells: two vehicles of one lane row are at least ceil(shortest length) cells
+// apart, so with every length above 3 m a granule of 4 cells never holds two of them and one code byte per
+// granule is enough (the kernel raises ERR_SPACING if it ever sees a closer pair).  TS_CODE_GRANULE=0 in
+// the environment keeps one byte per cell (a diagnostic: A/B timing and the parity tests of both layouts).
+static uint32_t code_granule_shift(const ts_params* prm) {
+    if (const char* e = std::getenv("TS_CODE_GRANULE")) if (e[0] == '0') return 0u;
+    float min_len = prm->n_types ? prm->type_len[0] : prm->veh_len;
+    for (uint32_t t = 1; t < prm->n_types && t < (uint32_t)kMaxTypes; t++) min_len = std::min(min_len, prm->type_len[t]);
+    return (min_len > 3.0f && prm->insert_clear_cells >= 4) ? 2u : 0u;
+}
 
 // Sizes only (what ts_query_workspace may look at).
 // `first_edge` (optional): receives each vehicle's first route edge, so that ts_create gathers
@@ -209,6 +224,7 @@ static int plan_sizes(const ts_network* net, const ts_routes* rt, const ts_param
     L.cap = (uint32_t)std::min<uint64_t>((uint64_t)L.V + std::max(q, L.Qcap) + 1024ull, 0x7FFFFFF0ull);
     L.emissions = prm->emissions ? 1u : 0u;
     L.typed = prm->n_types > 1 ? 1u : 0u;
+    L.cg = code_granule_shift(prm);
     L.ext = (prm->n_types != 0 || prm->amber_steps != 0) ? 1u : 0u;
     for (uint32_t h = 0; h < L.N && !L.ext; h++)
         if (net->node_ctrl[h] > TS_CTRL_SIGNAL) L.ext = 1u;
@@ -753,6 +769,7 @@ static void bind_ctx(ts_sim* s, const ts_params* p) {
     q.lc_pow2 = (p->lc_period && !(p->lc_period & (p->lc_period - 1))) ? 1u : 0u;
     q.lc_period = p->lc_period; q.insert_clear = p->insert_clear_cells; q.sample_period = p->sample_period_steps;
     q.inv_dt = 1.0f / p->dt;
+    q.cg = L.cg;
     for (int t = 0; t < kMaxTypes; t++) {
         const bool given = (uint32_t)t < p->n_types;
         const float len_t = given ? p->type_len[t] : p->veh_len, a_t = given ? p->type_a[t] : p->a;
@@ -1088,7 +1105,7 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             // The big size: 896 threads (28 warps, 72 registers) while the atlas is L2-resident; where its gathers
             // miss L2 (config 4: 460 MB) the spills of that size cost more than its warps bring and 768 threads
             // (24 warps, 85 registers) measured best: 14.43 against 14.13 (640) and 14.01 (896) G vehicle-updates/s.
-            const bool atlas_in_l2 = s->L.atlas_chunks * 144ull <= (unsigned long long)s->l2_bytes;
+            const bool atlas_in_l2 = s->L.atlas_chunks * (16ull + (128ull >> s->L.cg)) <= (unsigned long long)s->l2_bytes;
             const int big_threads = s->adaptive_big ? s->adaptive_big : atlas_in_l2 ? 896 : 768;
             const uint32_t chunk = s->adaptive_chunk;
             uint32_t k = s->k, cur = s->cur;
@@ -1177,6 +1194,7 @@ static const char* describe(uint32_t err) {
     if (err & ERR_CELL_CLASH) return "atlas audit failed: two vehicles in one lane cell, or a vehicle whose cell is not marked";
     if (err & ERR_SLOTS) return "slot overflow";
     if (err & ERR_NAN) return "a vehicle's position or speed is NaN, negative or infinite";
+    if (err & ERR_SPACING) return "two vehicles of one lane within one code granule (4 cells)";
     return "internal logic check failed";
 }
 

@@ -19,7 +19,9 @@
 //
 // The traffic atlas is two planes over the same rows.  A lane row is
 // `stride` chunks of 128 cells (one cell = one metre), zero-padded:
-//   code plane : one byte per cell, the occupant's speed code (valid only where occupied);
+//   code plane : the occupant's speed code (valid only where occupied), one byte per GRANULE of
+//                2^cg cells: 4 cells where vehicles are longer than 3 m (two vehicles of a lane are
+//                then never in one granule, see Params::cg), else one byte per cell;
 //   occupancy  : one bit per cell, 16 bytes per chunk, so that "check the following bytes" for a
 //                128-cell lookahead is two independent 16-byte loads and an __ffs instead of a
 //                chain of up to nine dependent loads.
@@ -34,7 +36,7 @@ constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 // CTRL_STOP: stop control with a persistent node owner (reading R34); CTRL_SIGNAL_NM:
 // one signal phase per movement (inbound edge, outbound edge) ("combination nm"; R35)
 enum : uint32_t { CTRL_FREE = 0, CTRL_PRIORITY = 1, CTRL_SIGNAL = 2, CTRL_STOP = 3, CTRL_SIGNAL_NM = 4 };
-enum : uint32_t { ERR_CELL_CLASH = 1, ERR_SLOTS = 2, ERR_LOGIC = 4, ERR_NAN = 8 };
+enum : uint32_t { ERR_CELL_CLASH = 1, ERR_SLOTS = 2, ERR_LOGIC = 4, ERR_NAN = 8, ERR_SPACING = 16 };
 // flags in Slots::A.w above the lane number: the vehicle takes part in the steps; has made its stop
 // at the STOP line of its edge; holds the STOP node at the tail of its edge; its type
 enum : uint32_t { ALIVE = 0x100u, STOPPED = 0x200u, OWNS = 0x400u, TYPE_SHIFT = 12, TYPE_MASK = 0x3000u };
@@ -97,6 +99,10 @@ struct Params {
     float two_b;           // 2*b (amber: go on iff v^2 > 2 b (C - x))
     float stop_dist, stop_speed;
     uint32_t amber;        // steps of amber after every green
+    // code plane (and type plane): one byte per 2^cg cells of a lane row.  cg = 2 where no two vehicles of a
+    // lane can sit within 4 cells of each other (every vehicle longer than 3 m, insert_clear >= 4: the
+    // no-overlap cap of E2 keeps a follower's cell at least ceil(length) below its leader's), else 0.
+    uint32_t cg;
 };
 // a sample is taken with the state after every sample_period-th step.
 __device__ __forceinline__ bool sample_step(const Params& p, uint32_t k) {
@@ -365,8 +371,8 @@ __device__ __forceinline__ int scan_behind(const uint4* occ, uint32_t row, int f
     }
     return -1;
 }
-__device__ __forceinline__ uint32_t code_at(const uint8_t* codes, uint32_t row, int cell) {
-    return __ldcg(codes + ((size_t)row << 7) + cell);
+__device__ __forceinline__ uint32_t code_at(const uint8_t* codes, uint32_t row, int cell, uint32_t cg) {
+    return __ldcg(codes + ((((size_t)row << 7) + cell) >> cg));
 }
 
 // Atlas cell address: the atlas holds < 2^32 cells (checked at ts_create), so (row, cell) packs
@@ -385,21 +391,21 @@ __device__ __forceinline__ void atlas_move(const Ctx& c, uint32_t gc_from, uint3
         if ((gc_from >> 5) == (gc_to >> 5)) atomicXor(occ32 + (gc_to >> 5), bf | bt);
         else { atomicAnd(occ32 + (gc_from >> 5), ~bf); atomicOr(occ32 + (gc_to >> 5), bt); }
     }
-    c.codes[gc_to] = (uint8_t)code;
+    c.codes[gc_to >> c.p.cg] = (uint8_t)code;
 }
 // extended rule set: the occupant's type travels with its speed code (`code_type` = code | type << 8)
 __device__ __forceinline__ void atlas_set_type(const Ctx& c, uint32_t gc, uint32_t code_type) {
-    if (c.types) c.types[gc] = (uint8_t)(code_type >> 8);
+    if (c.types) c.types[gc >> c.p.cg] = (uint8_t)(code_type >> 8);
 }
-__device__ __forceinline__ uint32_t type_at(const uint8_t* types, uint32_t row, int cell) {
-    return __ldcg(types + ((size_t)row << 7) + cell);
+__device__ __forceinline__ uint32_t type_at(const uint8_t* types, uint32_t row, int cell, uint32_t cg) {
+    return __ldcg(types + ((((size_t)row << 7) + cell) >> cg));
 }
 __device__ __forceinline__ void atlas_vacate(const Ctx& c, uint32_t gc) {
     atomicAnd(reinterpret_cast<uint32_t*>(c.occ) + (gc >> 5), ~(1u << (gc & 31)));
 }
 __device__ __forceinline__ void atlas_occupy(const Ctx& c, uint32_t gc, uint32_t code) {
     atomicOr(reinterpret_cast<uint32_t*>(c.occ) + (gc >> 5), 1u << (gc & 31));
-    c.codes[gc] = (uint8_t)code;
+    c.codes[gc >> c.p.cg] = (uint8_t)code;
 }
 
 __device__ __forceinline__ unsigned long long mix64(unsigned long long z) {

@@ -145,17 +145,20 @@ __device__ __forceinline__ uint4 vehicle_phase1(const Ctx& c, const Slots& S, ui
     // trip 4: speed codes (EXT: and types) of the vehicles found, and the route entry after the next edge
     uint32_t code_lead = 1, code_Lt = 1, code_F = 1, e3 = NONE32;
     uint32_t ty_lead = 0, ty_Lt = 0, ty_F = 0;
-    if (cL >= 0) code_lead = code_at(c.codes, row, cL);
-    else if (cL2 >= 0) code_lead = code_at(c.codes, row2, cL2);
-    if (cLt >= 0) code_Lt = code_at(c.codes, rowt, cLt);
-    if (cF >= 0) code_F = code_at(c.codes, rowt, cF);
+    if (cL >= 0) code_lead = code_at(c.codes, row, cL, p.cg);
+    else if (cL2 >= 0) code_lead = code_at(c.codes, row2, cL2, p.cg);
+    if (cLt >= 0) code_Lt = code_at(c.codes, rowt, cLt, p.cg);
+    if (cF >= 0) code_F = code_at(c.codes, rowt, cF, p.cg);
     if (EXT && c.types) {
-        if (cL >= 0) ty_lead = type_at(c.types, row, cL);
-        else if (cL2 >= 0) ty_lead = type_at(c.types, row2, cL2);
-        if (cLt >= 0) ty_Lt = type_at(c.types, rowt, cLt);
-        if (cF >= 0) ty_F = type_at(c.types, rowt, cF);
+        if (cL >= 0) ty_lead = type_at(c.types, row, cL, p.cg);
+        else if (cL2 >= 0) ty_lead = type_at(c.types, row2, cL2, p.cg);
+        if (cLt >= 0) ty_Lt = type_at(c.types, rowt, cLt, p.cg);
+        if (cF >= 0) ty_F = type_at(c.types, rowt, cF, p.cg);
     }
     if (may_leave && !last && sc.x + 2 < sc.y) e3 = __ldg(c.route_edges + sc.x + 2);
+
+    // the code plane's granule holds ONE vehicle: a leader closer than a granule would share a code byte
+    if (cL >= 0 && cL - ci < (1 << p.cg) && p.cg) atomicOr(&c.dyn->error, ERR_SPACING);
 
     // 2b gaps (E3): measured to the REAR of the vehicle ahead, i.e. with the leader's own length
     const float len_lead = EXT ? p.t_len[ty_lead & 3u] : p.len;

@@ -136,3 +136,20 @@ def test_renumbered_edges_morton_order():
     b = W.by_name("cfg4_small_morton")
     assert b["name"] == "cfg4_small_morton"
     _compare(b, 7200, 1, chunk=3600)
+
+
+def test_both_code_plane_layouts(monkeypatch):
+    """The code plane holds one byte per 4-cell granule where no two vehicles of a lane can come within
+    4 cells of each other (every vehicle longer than 3 m, insert_clear_cells >= 4), else one byte per cell
+    (DESIGN.md section 4).  Same results either way: the per-cell layout forced through the environment on
+    the signal grid with trucks, and short vehicles (2.5 m, standing 3 m apart) that select it themselves."""
+    b = W.with_trucks(small_signal_grid(), share=0.3)
+    monkeypatch.setenv("TS_CODE_GRANULE", "0")
+    _compare(b, b["steps"], 1)
+    _compare(b, 600, 0)
+    monkeypatch.delenv("TS_CODE_GRANULE")
+    g = small_signal_grid()
+    short = dict(g, params=dict(g["params"], veh_len=2.5, s0=0.5, insert_clear_cells=3))
+    _compare(short, short["steps"], 1)
+    tight = dict(g, params=dict(g["params"], veh_len=3.5, s0=0.25))      # granule layout, vehicles 4 cells apart in a queue
+    _compare(tight, tight["steps"], 1)
