@@ -43,7 +43,10 @@ typedef enum ts_status {
                            vehicle, lookahead not a multiple of 16, ... */
     TS_ENOMEM = -2,     /* workspace too small */
     TS_ECUDA = -3,      /* CUDA runtime error (or no device) */
-    TS_EINVARIANT = -4  /* device-side sticky flag: two vehicles scattered to one cell */
+    TS_EINVARIANT = -4  /* device-side sticky flag: two vehicles scattered to one cell; a position or
+                           speed that is NaN, negative or infinite; two vehicles of one lane closer
+                           than the 4-cell granule of the atlas's code plane (cannot happen under the
+                           rule set with vehicles longer than 3 m: it means the state is corrupt) */
 } ts_status;
 
 /* Node control types ("stop and traffic light signals"). */
