@@ -46,7 +46,7 @@ typedef enum ts_status {
     TS_EINVARIANT = -4  /* device-side sticky flag: two vehicles scattered to one cell; a position or
                            speed that is NaN, negative or infinite; two vehicles of one lane closer
                            than the 4-cell granule of the atlas's code plane (cannot happen under the
-                           rule set with vehicles longer than 3 m: it means the state is corrupt) */
+                           rule set with vehicles of 4 m or more: it means the state is corrupt) */
 } ts_status;
 
 /* Node control types ("stop and traffic light signals"). */

@@ -143,17 +143,21 @@ struct Layout {
     }
 };
 
-// The code plane's granule (Params::cg).  A follower's advance is capped at the gap to its leader's cell
-// minus the leader's length (E2, E3), a lane change needs that gap on both sides (G1, G2) and an entrant
-// needs `insert_clear` free cells: two vehicles of one lane row are at least ceil(shortest length) cells
-// apart, so with every length above 3 m a granule of 4 cells never holds two of them and one code byte per
-// granule is enough (the kernel raises ERR_SPACING if it ever sees a closer pair).  TS_CODE_GRANULE=0 in
-// the environment keeps one byte per cell (a diagnostic: A/B timing and the parity tests of both layouts).
+// The code plane's granule (Params::cg): one byte per 4 cells is enough where two vehicles of one lane row are
+// never less than 4 cells apart.  With L the shortest vehicle length: a follower's advance is capped at the gap to
+// its leader's CELL minus the leader's length (E2, E3), so its new cell is at most cL - ceil(L); a lane change needs
+// that gap to the target lane's leader (G1) and, to the lag vehicle F, x - L - (cF + 1) >= the most F can advance
+// in the step (G2), so F ends more than L behind the changer and their cells differ by more than L - 1; an entrant
+// needs `insert_clear` free cells and lands more than L short of the lane-change zone (R24).  L >= 4 m and
+// insert_clear >= 4 therefore keep any two cells of a lane at least 4 apart (all five configs: 5 m, 7 cells);
+// the kernel raises ERR_SPACING if a vehicle ever finds its leader closer.  Otherwise: one byte per cell.
+// TS_CODE_GRANULE=0 in the environment keeps one byte per cell regardless (a diagnostic: A/B timing and the
+// parity tests of both layouts).
 static uint32_t code_granule_shift(const ts_params* prm) {
     if (const char* e = std::getenv("TS_CODE_GRANULE")) if (e[0] == '0') return 0u;
     float min_len = prm->n_types ? prm->type_len[0] : prm->veh_len;
     for (uint32_t t = 1; t < prm->n_types && t < (uint32_t)kMaxTypes; t++) min_len = std::min(min_len, prm->type_len[t]);
-    return (min_len > 3.0f && prm->insert_clear_cells >= 4) ? 2u : 0u;
+    return (min_len >= 4.0f && prm->insert_clear_cells >= 4) ? 2u : 0u;
 }
 
 // Sizes only (what ts_query_workspace may look at).

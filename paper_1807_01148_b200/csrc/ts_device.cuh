@@ -20,7 +20,7 @@
 // The traffic atlas is two planes over the same rows.  A lane row is
 // `stride` chunks of 128 cells (one cell = one metre), zero-padded:
 //   code plane : the occupant's speed code (valid only where occupied), one byte per GRANULE of
-//                2^cg cells: 4 cells where vehicles are longer than 3 m (two vehicles of a lane are
+//                2^cg cells: 4 cells where vehicles are at least 4 m long (two vehicles of a lane are
 //                then never in one granule, see Params::cg), else one byte per cell;
 //   occupancy  : one bit per cell, 16 bytes per chunk, so that "check the following bytes" for a
 //                128-cell lookahead is two independent 16-byte loads and an __ffs instead of a
@@ -100,8 +100,8 @@ struct Params {
     float stop_dist, stop_speed;
     uint32_t amber;        // steps of amber after every green
     // code plane (and type plane): one byte per 2^cg cells of a lane row.  cg = 2 where no two vehicles of a
-    // lane can sit within 4 cells of each other (every vehicle longer than 3 m, insert_clear >= 4: the
-    // no-overlap cap of E2 keeps a follower's cell at least ceil(length) below its leader's), else 0.
+    // lane can sit within 4 cells of each other (every vehicle at least 4 m long, insert_clear >= 4: see
+    // code_granule_shift() in ts_api.cu), else 0.
     uint32_t cg;
 };
 // a sample is taken with the state after every sample_period-th step.

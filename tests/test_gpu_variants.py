@@ -140,7 +140,7 @@ def test_renumbered_edges_morton_order():
 
 def test_both_code_plane_layouts(monkeypatch):
     """The code plane holds one byte per 4-cell granule where no two vehicles of a lane can come within
-    4 cells of each other (every vehicle longer than 3 m, insert_clear_cells >= 4), else one byte per cell
+    4 cells of each other (every vehicle at least 4 m long, insert_clear_cells >= 4), else one byte per cell
     (DESIGN.md section 4).  Same results either way: the per-cell layout forced through the environment on
     the signal grid with trucks, and short vehicles (2.5 m, standing 3 m apart) that select it themselves."""
     b = W.with_trucks(small_signal_grid(), share=0.3)
@@ -151,5 +151,5 @@ def test_both_code_plane_layouts(monkeypatch):
     g = small_signal_grid()
     short = dict(g, params=dict(g["params"], veh_len=2.5, s0=0.5, insert_clear_cells=3))
     _compare(short, short["steps"], 1)
-    tight = dict(g, params=dict(g["params"], veh_len=3.5, s0=0.25))      # granule layout, vehicles 4 cells apart in a queue
+    tight = dict(g, params=dict(g["params"], veh_len=4.0, s0=0.25, insert_clear_cells=4))   # granule layout, queues 4 cells apart
     _compare(tight, tight["steps"], 1)

@@ -180,3 +180,43 @@ def test_validation_rejects_bad_input(cfg1):
     bad = dict(cfg1); bad["params"] = dict(cfg1["params"], lookahead_cells=100)
     with pytest.raises(OracleError):
         Oracle(bad)
+
+
+def _closest_cells(bundle, steps):
+    """Smallest difference between the cells (floor of x) of two vehicles of one lane over a run of the oracle."""
+    o = Oracle(bundle)
+    closest = 1 << 30
+    for _ in range(steps):
+        o.step(1, check=1)
+        st = o.read_state()
+        act = np.nonzero(st["status"] == 1)[0]
+        if act.size < 2:
+            continue
+        cell = np.floor(st["x"][act]).astype(np.int64)
+        key = st["edge"][act].astype(np.int64) * 16 + st["lane"][act]
+        order = np.lexsort((cell, key))
+        same = key[order][1:] == key[order][:-1]
+        if same.any():
+            closest = min(closest, int((cell[order][1:] - cell[order][:-1])[same].min()))
+    return closest, o.counters()
+
+
+def test_cells_of_one_lane_stay_a_vehicle_length_apart():
+    """What lets the CUDA atlas keep ONE speed-code byte per 4 cells: under the rule
+    set the cells of two vehicles of a lane differ by at least ceil(L) through following (E2 caps the advance
+    at the gap to the leader's cell minus its length), by more than L - 1 after a lane change with a lag
+    vehicle (G2), and entrants need insert_clear free cells -- so with L >= 4 m never less than 4.  Checked on
+    the oracle at every step of dense platoons with forced merges, a signalised grid with queues, trucks, and
+    a queue of 4 m vehicles standing 0.25 m apart."""
+    from test_oracle_lane_change_referee import _platoon_scenario
+    for politeness in (0.2, 0.5):
+        closest, cnt = _closest_cells(_platoon_scenario(politeness, 5), 1400)
+        assert cnt["lc_accepts"] > 100 and closest >= 5, (closest, cnt)
+    closest, cnt = _closest_cells(small_signal_grid(), 1500)
+    assert cnt["lc_accepts"] > 50 and closest >= 5, closest
+    closest, _ = _closest_cells(W.with_trucks(small_signal_grid(n_vehicles=900, steps=700), share=0.3), 700)
+    assert closest >= 5, closest
+    g = small_signal_grid()
+    tight = dict(g, params=dict(g["params"], veh_len=4.0, s0=0.25, insert_clear_cells=4))
+    closest, cnt = _closest_cells(tight, 1500)
+    assert 4 <= closest <= 5 and cnt["lc_accepts"] > 50, closest
