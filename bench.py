@@ -531,7 +531,7 @@ def main():
                    "sim_steps_per_bench_step": sim_steps, "vehicle_updates_per_bench_step": updates,
                    "start_step": args.start_step, "tuning": tuning, "emissions": bool(args.emissions), "phase_ns_per_sim_step": phase_ns,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "step_kernel": ("persistent cooperative, CTA size chosen on the device per 2048 steps (640 / 896 threads)" if adaptive
+                   "step_kernel": ("persistent cooperative, CTA size chosen on the device per 2048 steps (640 / 768 threads)" if adaptive
                                    else "persistent cooperative" if args.mode == 1 else "two launches per sim step"),
                    "l2": "flushed between timed iterations (256 MiB fill) and inputs (routes+atlas) exceed L2"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

@@ -349,13 +349,13 @@ int ts_sssp_static(uint32_t n_nodes, uint32_t n_edges, const uint32_t *d_out_off
  *                  the n steps with grid-wide barriers; 0 = one launch per phase.
  *  "threads"       CTA size of the persistent kernel (multiple of 32 in 64..1024).  Default: not
  *                  fixed -- ts_step enqueues every chunk of 2048 steps twice, with 640 threads
- *                  (spill-free; best while a step is one warp's latency) and with 896 -- 768 where the atlas exceeds L2 -- (more warps;
+ *                  (spill-free; best while a step is one warp's latency) and with 768 (more warps;
  *                  best once a CTA holds several rounds of vehicles), and the device runs the one
  *                  that fits the number of live slots; the other launch returns at once.  Setting
  *                  "threads" or "blocks_per_sm" (or "profile") fixes the size; "adaptive" 1 undoes it.
  *  "adaptive_chunk", "adaptive_above", "adaptive_big"  steps per chunk (default 2048), the number of live slots
  *                  above which the big size is preferred (default 640 per SM; -1 restores it), and the big
- *                  size itself (0 = the default: 896, or 768 where the atlas exceeds L2).
+ *                  size itself (0 = the default: 768).
  *  "blocks_per_sm" resident CTAs per SM of the persistent kernel (default 1).
  *  "sort_period"   steps between compaction of retired slots + re-sort of the live ones by
  *                  edge; 0 = never; default 128 (256 on networks

@@ -262,14 +262,14 @@ struct ts_sim {
     int blocks_per_sm = 1;
     uint32_t chunk_no = 0;    // adaptive chunks enqueued since ts_reset (parity selects Dyn::prefer_big[])
     uint32_t adaptive_chunk = 2048;   // steps per adaptive chunk
-    int adaptive_big = 0;             // CTA size of the big launch of a chunk; 0 = 896, or 768 where the atlas exceeds L2
+    int adaptive_big = 0;             // CTA size of the big launch of a chunk; 0 = 768
     // Most move-record tiles per thread kept in shared memory.  Shared memory and L1 are one 228 KB array: what the
     // move records do not take stays L1, which holds the edge records of the SM's vehicles across steps (the grid
     // barrier keeps L1 alive).  Records beyond the limit go through L2 (Ctx::mr_g).  Measured: config 4 (3 M slots:
     // the records would take all of it) 11.2 -> 14.1 G vehicle-updates/s, config 3 17.7 -> 18.0, config 5 3.72 -> 3.88.
     uint32_t smem_tiles = 6;
     long long adaptive_above = -1;    // live slots above which the big CTA size is preferred (-1: one round of tiles at 640 threads)
-    int adaptive = 1;         // no CTA size asked for: 640 threads, or 896 while more than one round of tiles is live
+    int adaptive = 1;         // no CTA size asked for: 640 threads, or 768 while more than one round of tiles is live
     int sms = 0;
     uint32_t sort_period = 128;  // steps between compaction + re-sort; 0 = never (set in ts_create)
     uint32_t profile = 0;
@@ -1102,15 +1102,15 @@ static int run_steps(ts_sim* s, uint32_t n, unsigned long long* d_digests) {
             if (sorts & 1) s->cur ^= 1;
         } else {
             // Adaptive CTA size without a host round trip: the steps go out in chunks, each chunk as
-            // TWO launches (640 threads, spill-free, best while a step is one warp's latency; 896
+            // TWO launches (640 threads, spill-free, best while a step is one warp's latency; 768
             // threads, more warps, best once CTAs hold several rounds of tiles); the device runs the
             // one the previous chunk asked for (Dyn::prefer_big) and the other returns at once.
             // Results do not depend on the launch geometry.
-            // The big size: 896 threads (28 warps, 72 registers) while the atlas is L2-resident; where its gathers
-            // miss L2 (config 4: 460 MB) the spills of that size cost more than its warps bring and 768 threads
-            // (24 warps, 85 registers) measured best: 14.43 against 14.13 (640) and 14.01 (896) G vehicle-updates/s.
-            const bool atlas_in_l2 = s->L.atlas_chunks * (16ull + (128ull >> s->L.cg)) <= (unsigned long long)s->l2_bytes;
-            const int big_threads = s->adaptive_big ? s->adaptive_big : atlas_in_l2 ? 896 : 768;
+            // The big size: 768 threads (24 warps, 80 registers).  Measured with the 4-cell code granule, G vehicle-updates/s
+            // at 704 / 736 / 768 / 800 / 832 / 896 / 960 / 1024: config 3 17.59 / 17.84 / 18.14 / 17.29 / 17.71 / 17.92 / 16.87 /
+            // 17.02; the dense diagnostic 21.53 / - / 21.81 / - / 21.55 / 21.77; config 4 14.65 (704) / 15.35 (768)
+            // (profiles/r02d_code_granule.md).  Until then it was 896 where the atlas fits L2.
+            const int big_threads = s->adaptive_big ? s->adaptive_big : 768;
             const uint32_t chunk = s->adaptive_chunk;
             uint32_t k = s->k, cur = s->cur;
             for (uint32_t done = 0; done < n;) {

@@ -65,7 +65,7 @@ def test_mixed_controls(mode):
     dict(sort_period=7, threads=128),          # several slots per thread, ragged tile tails
     dict(sort_period=50, threads=512, blocks_per_sm=2),
     dict(sort_period=3, threads=64),           # move records overflow shared memory into global
-    dict(adaptive_chunk=37, adaptive_above=0),     # adaptive CTA size: 896 threads from the second chunk on
+    dict(adaptive_chunk=37, adaptive_above=0),     # adaptive CTA size: the big size (768 threads) from the second chunk on
     dict(adaptive_chunk=50, adaptive_above=700),   # ... switching both ways as the slot count crosses 700
     dict(adaptive_chunk=1, adaptive_above=300, sort_period=5),
     dict(smem_tiles=0, threads=64, sort_period=16),    # every move record through L2
