@@ -12,7 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libts.so")
 SOURCES = ["ts_api.cu"]
-HEADERS = ["ts_device.cuh", "ts_phases.cuh", "ts_sort.cuh", os.path.join("..", "..", "include", "trafficsim.h")]
+HEADERS = ["ts_device.cuh", "ts_phases.cuh", "ts_sort.cuh", "ts_reroute.cuh", "ts_sue.cuh",
+           os.path.join("..", "..", "include", "trafficsim.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
