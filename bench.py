@@ -54,11 +54,11 @@ def measured_traffic(name, geometry):
     """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the step kernel over one whole
     run of workload `name`, from the committed ncu capture of every launch of the geometry the
     bench line was measured with (the same two metrics a --set full capture holds; one launch of it is
-    captured in full beside it) (profiles/r02d_kernel_traffic.csv:
+    captured in full beside it) (profiles/r02e_kernel_traffic.csv:
     workload,geometry,dram_read_bytes,dram_write_bytes,launches; geometry = "adaptive" -- the default:
     the sum over the launches of every 2048-step chunk -- or "threadsNNN").  None if that geometry
     was not captured: a number from another geometry is not this run's traffic."""
-    path = os.path.join(ROOT, "profiles", "r02d_kernel_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r02e_kernel_traffic.csv")
     try:
         for line in open(path):
             f = [t.strip() for t in line.split(",")]
@@ -520,7 +520,7 @@ def main():
     geometry = "adaptive" if adaptive else f"threads{args.threads or 640}"
     traffic = (measured_traffic(args.workload, geometry)
                if args.mode == 1 and not args.start_step and not args.sim_steps and not args.emissions else None)
-    traffic_src = (f"ncu dram__bytes_read.sum + dram__bytes_write.sum, every launch of one whole run, geometry {geometry} (profiles/r02d_kernel_traffic.csv)" if traffic is not None
+    traffic_src = (f"ncu dram__bytes_read.sum + dram__bytes_write.sum, every launch of one whole run, geometry {geometry} (profiles/r02e_kernel_traffic.csv)" if traffic is not None
                    else f"no ncu capture of geometry {geometry} for this workload")
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
