@@ -91,7 +91,7 @@ struct Layout {
     uint32_t n_src = 0, Qcap = 0;
     size_t rr_routes2, rr_end, rr_origin, rr_dest, rr_srcidx, rr_mask, rr_newlen, rr_newoff, rr_bsum, rr_first2,
         rr_out_off, rr_out_edge, rr_efrom, rr_eto, rr_w, rr_wfree, rr_src, rr_todo, rr_pred, rr_lab, rr_fa, rr_fb,
-        rr_stamp, rr_err;
+        rr_stamp, rr_err, rr_adjw;
     static constexpr uint32_t kDigestChunk = 8192;
     size_t take(size_t bytes) {
         size_t off = total;
@@ -139,6 +139,7 @@ struct Layout {
             rr_pred = take((size_t)n_src * N * 4);
             rr_lab = take((size_t)kRrCtas * N * 8); rr_fa = take((size_t)kRrCtas * N * 4); rr_fb = take((size_t)kRrCtas * N * 4);
             rr_stamp = take((size_t)kRrCtas * N * 4); rr_err = take(4);
+            rr_adjw = take((size_t)E * 16);
         }
     }
 };
@@ -993,6 +994,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         r.first2 = at<uint32_t>(s, L.rr_first2); r.pred = at<uint32_t>(s, L.rr_pred);
         r.lab = at<unsigned long long>(s, L.rr_lab); r.fa = at<uint32_t>(s, L.rr_fa); r.fb = at<uint32_t>(s, L.rr_fb);
         r.stamp = at<uint32_t>(s, L.rr_stamp); r.error = at<uint32_t>(s, L.rr_err);
+        r.adjw = at<uint4>(s, L.rr_adjw);
     }
     // the staging vectors die with this scope: make sure the copies have left them
     lap("enqueue copies, host copies");
@@ -1362,8 +1364,10 @@ extern "C" int ts_reroute(ts_sim* s, const uint32_t* w_free, const uint8_t* mask
     for (auto& e : ev) CUDA_TRY(cudaEventCreate(&e));
     k_rr_weights<<<std::max(1u, std::min(1184u, (E + 255) / 256)), 256, 0, st>>>(r);
     CUDA_TRY(cudaEventRecord(ev[0], st));
-    if (!todo.empty())
+    if (!todo.empty()) {
+        k_rr_pack<<<std::max(1u, std::min(1184u, (E + 255) / 256)), 256, 0, st>>>(r);
         k_rr_sssp<<<std::min<uint32_t>(kRrCtas, (uint32_t)todo.size()), kRrThreads, 0, st>>>(r, at<uint32_t>(s, L.rr_todo), (uint32_t)todo.size());
+    }
     CUDA_TRY(cudaEventRecord(ev[1], st));
     const uint32_t vb = std::max(1u, std::min(1184u, (V + 255) / 256));
     k_rr_len<<<vb, 256, 0, st>>>(r);
@@ -1447,7 +1451,7 @@ extern "C" int ts_read_routes(ts_sim* s, uint64_t* route_off, uint32_t* route_ed
 
 struct SueLayout {
     size_t total = 0;
-    size_t out_off, out_edge, efrom, eto, t0, cap, x, t, w, y, part, od_o, od_d, od_t, od_s, src, todo, pred, lab, fa, fb, stamp, err;
+    size_t out_off, out_edge, efrom, eto, t0, cap, x, t, w, y, part, od_o, od_d, od_t, od_s, src, todo, pred, lab, fa, fb, stamp, err, adjw;
     uint32_t n_src = 0;
     size_t take(size_t bytes) { size_t off = total; total += (bytes + 255) & ~(size_t)255; return off; }
     void plan(uint32_t N, uint32_t E, uint32_t n_od) {
@@ -1458,6 +1462,7 @@ struct SueLayout {
         src = take((size_t)n_src * 4); todo = take((size_t)n_src * 4); pred = take((size_t)n_src * N * 4);
         lab = take((size_t)kRrCtas * N * 8); fa = take((size_t)kRrCtas * N * 4); fb = take((size_t)kRrCtas * N * 4);
         stamp = take((size_t)kRrCtas * N * 4); err = take(4);
+        adjw = take((size_t)E * 16);
     }
 };
 
@@ -1529,7 +1534,7 @@ extern "C" int ts_sue_solve(const ts_sue_problem* p, const ts_device* dev, ts_su
     r.out_off = up32(L.out_off); r.out_edge = up32(L.out_edge); r.edge_from = up32(L.efrom); r.edge_to = up32(L.eto);
     r.w = up32(L.w); r.src_node = up32(L.src); r.pred = up32(L.pred);
     r.lab = reinterpret_cast<unsigned long long*>(ws + L.lab); r.fa = up32(L.fa); r.fb = up32(L.fb); r.stamp = up32(L.stamp);
-    r.error = up32(L.err);
+    r.error = up32(L.err); r.adjw = reinterpret_cast<uint4*>(ws + L.adjw);
     unsigned long long* y = reinterpret_cast<unsigned long long*>(ws + L.y);
     const uint32_t eb = std::max(1u, std::min(1184u, (E + 255) / 256)), ob = std::max(1u, std::min(1184u, (n_od + 255) / 256));
     cudaEvent_t ev0, ev1, t0e, t1e;
@@ -1540,7 +1545,10 @@ extern "C" int ts_sue_solve(const ts_sue_problem* p, const ts_device* dev, ts_su
     auto assign = [&](const double* x) -> int {
         k_sue_times<<<eb, 256, 0, st>>>(E, dp(L.t0), dp(L.cap), x, p->alpha, p->weight_scale, dp(L.t), r.w);
         CUDA_TRY(cudaEventRecord(t0e, st));
-        if (L.n_src) k_rr_sssp<<<std::min<uint32_t>(kRrCtas, L.n_src), kRrThreads, 0, st>>>(r, up32(L.todo), L.n_src);
+        if (L.n_src) {
+            k_rr_pack<<<eb, 256, 0, st>>>(r);
+            k_rr_sssp<<<std::min<uint32_t>(kRrCtas, L.n_src), kRrThreads, 0, st>>>(r, up32(L.todo), L.n_src);
+        }
         CUDA_TRY(cudaEventRecord(t1e, st));
         CUDA_TRY(cudaMemsetAsync(y, 0, (size_t)E * 8, st));
         if (n_od) k_sue_aon<<<ob, 256, 0, st>>>(n_od, up32(L.od_o), up32(L.od_d), up32(L.od_t), up32(L.od_s), r.pred, N, r.edge_from, y);
@@ -1621,7 +1629,8 @@ constexpr uint32_t kStaticMaxNodes = 65536;                        // 20 bytes o
 constexpr uint32_t kStaticBytesPerNode = 20;
 static __device__ __align__(256) unsigned char g_sssp_scratch[kStaticScratchBytes];
 
-// Same relaxation as k_rr_sssp (ts_reroute.cuh), trees numbered 0..n_src-1 in the caller's source order;
+// Same relaxation rule as k_rr_sssp (ts_reroute.cuh; one outbound edge at a time here, four at a time there: the
+// labels at the end are the same minimum), trees numbered 0..n_src-1 in the caller's source order;
 // `scratch` is the device address of g_sssp_scratch (device code could name the array directly, the host cannot).
 __global__ void __launch_bounds__(kRrThreads) k_sssp_static(unsigned char* scratch, uint32_t N, const uint32_t* __restrict__ out_off,
                                                             const uint32_t* __restrict__ out_edge, const uint32_t* __restrict__ edge_to,

@@ -9,6 +9,7 @@
 //
 // Kernels (product code, sm_100a; shares nothing with oracle/reroute.py):
 //   k_rr_weights   w[e] = round-half-up(256 * exit_steps_sum / exited), else the caller's free-flow weight
+//   k_rr_pack      per outbound edge in CSR order { edge id, head node, weight }: one load per relaxation
 //   k_rr_sssp      one CTA of 256 threads per origin node, 592 in flight: label-correcting shortest paths over the CSR of outbound
 //                  edges, frontier by frontier; a node's label is ONE 64-bit word (distance << 32 |
 //                  inbound edge) under atomicMin, so the lexicographic minimum IS the tie-break rule
@@ -37,6 +38,7 @@ struct RrCtx {
     const uint32_t* edge_from;     // [E]
     const uint32_t* edge_to;       // [E]
     uint32_t* w;                   // [E]   routing weights of this call
+    uint4* adjw;                   // [E]   by CSR position: { edge id, head node, weight of this call, - } (k_rr_pack)
     const uint32_t* w_free;        // [E]   the caller's free-flow weights
     // measurements (the step kernels' accumulators)
     const uint32_t* st_exited;
@@ -73,6 +75,15 @@ __global__ void k_rr_weights(const RrCtx r) {
     }
 }
 
+// What a relaxation needs of an outbound edge, side by side in CSR order: one 16-byte load instead of the edge id
+// followed by its head node and weight (a dependent trip to L2 less per frontier).  Run before every k_rr_sssp.
+__global__ void k_rr_pack(const RrCtx r) {
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < r.E; j += gridDim.x * blockDim.x) {
+        const uint32_t e = r.out_edge[j];
+        r.adjw[j] = make_uint4(e, r.edge_to[e], r.w[e], 0u);
+    }
+}
+
 // todo[0..n_todo): indices into src_node of the trees wanted.
 __global__ void __launch_bounds__(kRrThreads) k_rr_sssp(const RrCtx r, const uint32_t* __restrict__ todo, uint32_t n_todo) {
     __shared__ uint32_t sh_next;
@@ -94,16 +105,33 @@ __global__ void __launch_bounds__(kRrThreads) k_rr_sssp(const RrCtx r, const uin
                 const uint32_t u = __ldcg(fa + i);
                 const unsigned long long du = __ldcg(lab + u) >> 32;
                 const uint32_t j1 = r.out_off[u + 1];
-                for (uint32_t j = r.out_off[u]; j < j1; j++) {
-                    const uint32_t e = r.out_edge[j], v = r.edge_to[e];
-                    const unsigned long long nd = du + r.w[e];
-                    if (nd >= 0xFFFFFFFFull) { *r.error = 1u; continue; }
-                    const unsigned long long cand = (nd << 32) | e;
-                    const unsigned long long old = atomicMin(lab + v, cand);
+                // the outbound edges of u four at a time, every load of a stage issued before any is consumed: a
+                // relaxation is a chain of dependent trips to L2 (edge record -> atomicMin -> stamp), and one after the other they were what a frontier took (a node of a road network has 3-4
+                // outbound edges).  Same labels at the end: the minimum does not depend on the order of the attempts.
+                for (uint32_t j = r.out_off[u]; j < j1; j += 4) {
+                    uint4 a[4];                                   // { edge id, head node, weight, - }
+                    unsigned long long cand[4], old[4];
+                    bool go[4];
+#pragma unroll
+                    for (int q = 0; q < 4; q++) { go[q] = j + q < j1; if (go[q]) a[q] = r.adjw[j + q]; }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q]) {
+                        const unsigned long long nd = du + a[q].z;
+                        if (nd >= 0xFFFFFFFFull) { *r.error = 1u; go[q] = false; }
+                        cand[q] = (nd << 32) | a[q].x;
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q]) old[q] = atomicMin(lab + a[q].y, cand[q]);
                     // a shorter distance: v's outbound edges must be relaxed again.  (The same distance over
                     // a lower edge id only replaces the inbound edge.)
-                    if (cand < old && nd < (old >> 32) && atomicExch(stamp + v, epoch) != epoch)
-                        fb[atomicAdd(&sh_next, 1u)] = v;
+                    uint32_t seen[4];
+#pragma unroll
+                    for (int q = 0; q < 4; q++) {
+                        go[q] = go[q] && cand[q] < old[q] && (cand[q] >> 32) < (old[q] >> 32);
+                        if (go[q]) seen[q] = atomicExch(stamp + a[q].y, epoch);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q] && seen[q] != epoch) fb[atomicAdd(&sh_next, 1u)] = a[q].y;
                 }
             }
             __syncthreads();
