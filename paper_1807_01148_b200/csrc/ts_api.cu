@@ -137,9 +137,9 @@ struct Layout {
             rr_efrom = take((size_t)E * 4); rr_eto = take((size_t)E * 4); rr_w = take((size_t)E * 4); rr_wfree = take((size_t)E * 4);
             rr_src = take((size_t)n_src * 4); rr_todo = take((size_t)n_src * 4);
             rr_pred = take((size_t)n_src * N * 4);
-            rr_lab = take((size_t)kRrCtas * N * 8); rr_fa = take((size_t)kRrCtas * N * 4); rr_fb = take((size_t)kRrCtas * N * 4);
+            rr_lab = take((size_t)kRrCtas * N * 8); rr_fa = take((size_t)kRrCtas * N * 8); rr_fb = take((size_t)kRrCtas * N * 8);
             rr_stamp = take((size_t)kRrCtas * N * 4); rr_err = take(4);
-            rr_adjw = take((size_t)E * 16);
+            rr_adjw = take(((size_t)E + 4) * 16);
         }
     }
 };
@@ -992,7 +992,7 @@ extern "C" int ts_create(const ts_network* net, const ts_routes* rt, const ts_de
         r.src_node = at<uint32_t>(s, L.rr_src); r.mask = at<uint8_t>(s, L.rr_mask);
         r.new_len = at<uint32_t>(s, L.rr_newlen); r.new_off = at<uint32_t>(s, L.rr_newoff); r.block_sum = at<uint32_t>(s, L.rr_bsum);
         r.first2 = at<uint32_t>(s, L.rr_first2); r.pred = at<uint32_t>(s, L.rr_pred);
-        r.lab = at<unsigned long long>(s, L.rr_lab); r.fa = at<uint32_t>(s, L.rr_fa); r.fb = at<uint32_t>(s, L.rr_fb);
+        r.lab = at<unsigned long long>(s, L.rr_lab); r.fa = at<uint2>(s, L.rr_fa); r.fb = at<uint2>(s, L.rr_fb);
         r.stamp = at<uint32_t>(s, L.rr_stamp); r.error = at<uint32_t>(s, L.rr_err);
         r.adjw = at<uint4>(s, L.rr_adjw);
     }
@@ -1460,9 +1460,9 @@ struct SueLayout {
         w = take((size_t)E * 4); y = take((size_t)E * 8); part = take((size_t)kSueBlocks * 2 * 8);
         od_o = take((size_t)n_od * 4); od_d = take((size_t)n_od * 4); od_t = take((size_t)n_od * 4); od_s = take((size_t)n_od * 4);
         src = take((size_t)n_src * 4); todo = take((size_t)n_src * 4); pred = take((size_t)n_src * N * 4);
-        lab = take((size_t)kRrCtas * N * 8); fa = take((size_t)kRrCtas * N * 4); fb = take((size_t)kRrCtas * N * 4);
+        lab = take((size_t)kRrCtas * N * 8); fa = take((size_t)kRrCtas * N * 8); fb = take((size_t)kRrCtas * N * 8);
         stamp = take((size_t)kRrCtas * N * 4); err = take(4);
-        adjw = take((size_t)E * 16);
+        adjw = take(((size_t)E + 4) * 16);
     }
 };
 
@@ -1470,6 +1470,7 @@ static int sue_plan(const ts_sue_problem* p, SueLayout& L, std::vector<uint32_t>
     if (!p || !p->edge_from || !p->edge_to || !p->t0 || !p->cap || (p->n_od && (!p->od_origin || !p->od_dest || !p->od_trips)))
         return fail(TS_EINVAL, "null argument");
     if (p->n_nodes == 0 || p->n_edges == 0) return fail(TS_EINVAL, "empty network");
+    if (p->n_edges >= 0x80000000u) return fail(TS_EINVAL, "more than 2^31 edges");
     if (!(p->alpha >= 0) || !(p->weight_scale > 0) || p->bisections > 64) return fail(TS_EINVAL, "alpha >= 0, weight_scale > 0, bisections <= 64");
     for (uint32_t e = 0; e < p->n_edges; e++) {
         if (p->edge_from[e] >= p->n_nodes || p->edge_to[e] >= p->n_nodes) return fail(TS_EINVAL, "edge %u: endpoint out of range", e);
@@ -1533,7 +1534,7 @@ extern "C" int ts_sue_solve(const ts_sue_problem* p, const ts_device* dev, ts_su
     r.N = N; r.E = E; r.n_src = L.n_src;
     r.out_off = up32(L.out_off); r.out_edge = up32(L.out_edge); r.edge_from = up32(L.efrom); r.edge_to = up32(L.eto);
     r.w = up32(L.w); r.src_node = up32(L.src); r.pred = up32(L.pred);
-    r.lab = reinterpret_cast<unsigned long long*>(ws + L.lab); r.fa = up32(L.fa); r.fb = up32(L.fb); r.stamp = up32(L.stamp);
+    r.lab = reinterpret_cast<unsigned long long*>(ws + L.lab); r.fa = reinterpret_cast<uint2*>(ws + L.fa); r.fb = reinterpret_cast<uint2*>(ws + L.fb); r.stamp = up32(L.stamp);
     r.error = up32(L.err); r.adjw = reinterpret_cast<uint4*>(ws + L.adjw);
     unsigned long long* y = reinterpret_cast<unsigned long long*>(ws + L.y);
     const uint32_t eb = std::max(1u, std::min(1184u, (E + 255) / 256)), ob = std::max(1u, std::min(1184u, (n_od + 255) / 256));

@@ -9,7 +9,7 @@
 //
 // Kernels (product code, sm_100a; shares nothing with oracle/reroute.py):
 //   k_rr_weights   w[e] = round-half-up(256 * exit_steps_sum / exited), else the caller's free-flow weight
-//   k_rr_pack      per outbound edge in CSR order { edge id, head node, weight }: one load per relaxation
+//   k_rr_pack      per outbound edge in CSR order { edge id, head node, weight, where the head's records start }
 //   k_rr_sssp      one CTA of 256 threads per origin node, 592 in flight: label-correcting shortest paths over the CSR of outbound
 //                  edges, frontier by frontier; a node's label is ONE 64-bit word (distance << 32 |
 //                  inbound edge) under atomicMin, so the lexicographic minimum IS the tie-break rule
@@ -38,7 +38,7 @@ struct RrCtx {
     const uint32_t* edge_from;     // [E]
     const uint32_t* edge_to;       // [E]
     uint32_t* w;                   // [E]   routing weights of this call
-    uint4* adjw;                   // [E]   by CSR position: { edge id, head node, weight of this call, - } (k_rr_pack)
+    uint4* adjw;                   // [E+4] by CSR position: one record per outbound edge (k_rr_pack)
     const uint32_t* w_free;        // [E]   the caller's free-flow weights
     // measurements (the step kernels' accumulators)
     const uint32_t* st_exited;
@@ -60,7 +60,7 @@ struct RrCtx {
     // trees
     uint32_t* pred;                // [n_src][N] inbound edge on the shortest path from the source, kRrNone = none
     unsigned long long* lab;       // [kRrCtas][N] labels of the trees in flight
-    uint32_t* fa; uint32_t* fb;    // [kRrCtas][N] frontiers
+    uint2* fa; uint2* fb;          // [kRrCtas][N] frontiers: { node, CSR position of its first outbound edge }
     uint32_t* stamp;               // [kRrCtas][N] last frontier a node was put in
     uint32_t* error;               // sticky: 1 = a path cost passed 2^32
 };
@@ -75,70 +75,83 @@ __global__ void k_rr_weights(const RrCtx r) {
     }
 }
 
-// What a relaxation needs of an outbound edge, side by side in CSR order: one 16-byte load instead of the edge id
-// followed by its head node and weight (a dependent trip to L2 less per frontier).  Run before every k_rr_sssp.
+// What a relaxation needs of an outbound edge, side by side in CSR order -- one 16-byte record instead of the edge id
+// followed by its head node and weight:
+//   { edge id | kRrLast on the last outbound edge of its tail node, head node, weight of this call,
+//     CSR position of the HEAD node's first outbound edge (kRrNone if it has none) }
+// The last word lets a frontier entry carry where its node's records start, so that a node's label and its records
+// are fetched in the same trip.  Edge ids stay below 2^31.  Run before every k_rr_sssp.
+constexpr uint32_t kRrLast = 0x80000000u;
 __global__ void k_rr_pack(const RrCtx r) {
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < r.E; j += gridDim.x * blockDim.x) {
-        const uint32_t e = r.out_edge[j];
-        r.adjw[j] = make_uint4(e, r.edge_to[e], r.w[e], 0u);
+        const uint32_t e = r.out_edge[j], u = r.edge_from[e], v = r.edge_to[e];
+        const uint32_t hv = r.out_off[v] < r.out_off[v + 1] ? r.out_off[v] : kRrNone;
+        r.adjw[j] = make_uint4(e | (j + 1 == r.out_off[u + 1] ? kRrLast : 0u), v, r.w[e], hv);
     }
 }
 
 // todo[0..n_todo): indices into src_node of the trees wanted.
+// Frontier entries are { node, CSR position of its first outbound edge }; fa / fb hold N of them per tree in flight.
 __global__ void __launch_bounds__(kRrThreads) k_rr_sssp(const RrCtx r, const uint32_t* __restrict__ todo, uint32_t n_todo) {
     __shared__ uint32_t sh_next;
     const uint32_t t = threadIdx.x, T = blockDim.x, N = r.N;
     unsigned long long* lab = r.lab + (size_t)blockIdx.x * N;
     uint32_t* stamp = r.stamp + (size_t)blockIdx.x * N;
-    uint32_t* fa = r.fa + (size_t)blockIdx.x * N;
-    uint32_t* fb = r.fb + (size_t)blockIdx.x * N;
+    uint2* fa = r.fa + (size_t)blockIdx.x * N;
+    uint2* fb = r.fb + (size_t)blockIdx.x * N;
     for (uint32_t si = blockIdx.x; si < n_todo; si += gridDim.x) {
         const uint32_t s_idx = todo[si], s = r.src_node[s_idx];
         for (uint32_t v = t; v < N; v += T) { lab[v] = ~0ull; stamp[v] = 0u; }
         __syncthreads();
-        if (t == 0) { lab[s] = (unsigned long long)kRrNone; fa[0] = s; sh_next = 0; }   // distance 0, no inbound edge
+        const uint32_t s_first = r.out_off[s] < r.out_off[s + 1] ? r.out_off[s] : kRrNone;
+        if (t == 0) { lab[s] = (unsigned long long)kRrNone; fa[0] = make_uint2(s, s_first); sh_next = 0; }   // distance 0, no inbound edge
         __syncthreads();
-        uint32_t n_f = 1, epoch = 0;
+        uint32_t n_f = s_first != kRrNone ? 1u : 0u, epoch = 0;
         while (n_f) {
             epoch++;
             for (uint32_t i = t; i < n_f; i += T) {
-                const uint32_t u = __ldcg(fa + i);
-                const unsigned long long du = __ldcg(lab + u) >> 32;
-                const uint32_t j1 = r.out_off[u + 1];
-                // the outbound edges of u four at a time, every load of a stage issued before any is consumed: a
-                // relaxation is a chain of dependent trips to L2 (edge record -> atomicMin -> stamp), and one after the other they were what a frontier took (a node of a road network has 3-4
-                // outbound edges).  Same labels at the end: the minimum does not depend on the order of the attempts.
-                for (uint32_t j = r.out_off[u]; j < j1; j += 4) {
-                    uint4 a[4];                                   // { edge id, head node, weight, - }
+                const uint2 ent = __ldcg(fa + i);
+                // The outbound edges of the node four at a time, every load of a stage issued before any is
+                // consumed: a frontier is a chain of dependent trips to L2 (entry -> label and edge records ->
+                // atomicMin -> stamp), and edge after edge they were what a tree took (a node of a road network has
+                // 3-4 outbound edges).  Same labels at the end: the minimum does not depend on the order of the
+                // attempts.  Records read beyond the node's last one are ignored (adjw has 4 spare records).
+                const unsigned long long du = __ldcg(lab + ent.x) >> 32;
+                bool more = true;
+                for (uint32_t j = ent.y; more; j += 4) {
+                    uint4 a[4];
                     unsigned long long cand[4], old[4];
                     bool go[4];
 #pragma unroll
-                    for (int q = 0; q < 4; q++) { go[q] = j + q < j1; if (go[q]) a[q] = r.adjw[j + q]; }
+                    for (int q = 0; q < 4; q++) a[q] = r.adjw[j + q];
 #pragma unroll
-                    for (int q = 0; q < 4; q++) if (go[q]) {
+                    for (int q = 0; q < 4; q++) {
+                        go[q] = more;
+                        if (a[q].x & kRrLast) more = false;
                         const unsigned long long nd = du + a[q].z;
-                        if (nd >= 0xFFFFFFFFull) { *r.error = 1u; go[q] = false; }
-                        cand[q] = (nd << 32) | a[q].x;
+                        if (go[q] && nd >= 0xFFFFFFFFull) { *r.error = 1u; go[q] = false; }
+                        cand[q] = (nd << 32) | (a[q].x & ~kRrLast);
                     }
 #pragma unroll
                     for (int q = 0; q < 4; q++) if (go[q]) old[q] = atomicMin(lab + a[q].y, cand[q]);
                     // a shorter distance: v's outbound edges must be relaxed again.  (The same distance over
-                    // a lower edge id only replaces the inbound edge.)
+                    // a lower edge id only replaces the inbound edge.)  A head node without outbound edges has
+                    // nothing to relax and stays out of the frontier.
                     uint32_t seen[4];
 #pragma unroll
                     for (int q = 0; q < 4; q++) {
-                        go[q] = go[q] && cand[q] < old[q] && (cand[q] >> 32) < (old[q] >> 32);
+                        go[q] = go[q] && cand[q] < old[q] && (cand[q] >> 32) < (old[q] >> 32) && a[q].w != kRrNone;
                         if (go[q]) seen[q] = atomicExch(stamp + a[q].y, epoch);
                     }
 #pragma unroll
-                    for (int q = 0; q < 4; q++) if (go[q] && seen[q] != epoch) fb[atomicAdd(&sh_next, 1u)] = a[q].y;
+                    for (int q = 0; q < 4; q++) if (go[q] && seen[q] != epoch) fb[atomicAdd(&sh_next, 1u)] = make_uint2(a[q].y, a[q].w);
                 }
             }
             __syncthreads();
             n_f = sh_next;
             __syncthreads();
             if (t == 0) sh_next = 0;
-            uint32_t* tmp = fa; fa = fb; fb = tmp;
+            uint2* tmp = fa; fa = fb; fb = tmp;
             __threadfence_block();
             __syncthreads();
         }
