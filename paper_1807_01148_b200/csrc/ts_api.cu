@@ -1630,7 +1630,7 @@ constexpr uint32_t kStaticMaxNodes = 65536;                        // 20 bytes o
 constexpr uint32_t kStaticBytesPerNode = 20;
 static __device__ __align__(256) unsigned char g_sssp_scratch[kStaticScratchBytes];
 
-// Same relaxation rule as k_rr_sssp (ts_reroute.cuh; one outbound edge at a time here, four at a time there: the
+// Same relaxation rule as k_rr_sssp (ts_reroute.cuh; from the caller's CSR arrays here, from packed records there: the
 // labels at the end are the same minimum), trees numbered 0..n_src-1 in the caller's source order;
 // `scratch` is the device address of g_sssp_scratch (device code could name the array directly, the host cannot).
 __global__ void __launch_bounds__(kRrThreads) k_sssp_static(unsigned char* scratch, uint32_t N, const uint32_t* __restrict__ out_off,
@@ -1657,14 +1657,31 @@ __global__ void __launch_bounds__(kRrThreads) k_sssp_static(unsigned char* scrat
                 const uint32_t u = __ldcg(fa + i);
                 const unsigned long long du = __ldcg(lab + u) >> 32;
                 const uint32_t j1 = out_off[u + 1];
-                for (uint32_t j = out_off[u]; j < j1; j++) {
-                    const uint32_t e = out_edge[j], v = edge_to[e];
-                    const unsigned long long nd = du + w[e];
-                    if (nd >= 0xFFFFFFFFull) { if (error) *error = 1u; continue; }
-                    const unsigned long long cand = (nd << 32) | e;
-                    const unsigned long long old = atomicMin(lab + v, cand);
-                    if (cand < old && nd < (old >> 32) && atomicExch(stamp + v, epoch) != epoch)
-                        fb[atomicAdd(&sh_next, 1u)] = v;
+                // four outbound edges at a time, every load of a stage issued before any is consumed (k_rr_sssp
+                // does the same from packed records, which this call has no scratch for)
+                for (uint32_t j = out_off[u]; j < j1; j += 4) {
+                    uint32_t e[4], v[4], we[4], seen[4];
+                    unsigned long long cand[4], old[4];
+                    bool go[4];
+#pragma unroll
+                    for (int q = 0; q < 4; q++) { go[q] = j + q < j1; e[q] = go[q] ? out_edge[j + q] : 0u; }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q]) { v[q] = edge_to[e[q]]; we[q] = w[e[q]]; }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q]) {
+                        const unsigned long long nd = du + we[q];
+                        if (nd >= 0xFFFFFFFFull) { if (error) *error = 1u; go[q] = false; }
+                        cand[q] = (nd << 32) | e[q];
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q]) old[q] = atomicMin(lab + v[q], cand[q]);
+#pragma unroll
+                    for (int q = 0; q < 4; q++) {
+                        go[q] = go[q] && cand[q] < old[q] && (cand[q] >> 32) < (old[q] >> 32);
+                        if (go[q]) seen[q] = atomicExch(stamp + v[q], epoch);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; q++) if (go[q] && seen[q] != epoch) fb[atomicAdd(&sh_next, 1u)] = v[q];
                 }
             }
             __syncthreads();
