@@ -191,7 +191,10 @@ int ts_query_workspace(const ts_network *net, const ts_routes *routes,
  * ts_query_workspace says), TS_ECUDA (no device: there is no CPU fallback).
  * The host work (validation, departure-queue index) runs on up to 16 threads; the copy of the route table, the
  * largest input, is enqueued first and overlaps it when the caller's buffer is pinned.  With the environment
- * variable TS_TRACE_CREATE set, the milliseconds of each stage go to stderr. */
+ * variable TS_TRACE_CREATE set, the milliseconds of each stage go to stderr.
+ * Layout of the atlas: one occupancy bit per cell and one speed-code byte per 4 cells when every vehicle length is
+ * >= 4 m and insert_clear_cells >= 4 (two vehicles of a lane then never share 4 cells), else one byte per cell; the
+ * environment variable TS_CODE_GRANULE=0 forces the latter (a diagnostic; results are the same, the workspace larger). */
 int ts_create(const ts_network *net, const ts_routes *routes, const ts_departures *dep,
               const ts_params *params, const ts_device *dev, ts_sim **out);
 

@@ -49,6 +49,22 @@ def test_emission_totals_are_paid_for_only_when_asked(cfg1):
     assert plain + 8 * V + 16 * V <= with_totals <= plain + 8 * V + 16 * slots + 512
 
 
+def test_code_plane_granule_follows_the_vehicle_lengths(cfg1, monkeypatch):
+    """the atlas keeps one speed-code byte per 4 cells where every vehicle is at least 4 m long
+    and insert_clear_cells >= 4, one per cell otherwise (and when TS_CODE_GRANULE=0 asks for it).  Seen from outside
+    as the size of the workspace: config 1 has 96 lane rows of 2 chunks of 128 cells."""
+    from paper_1807_01148_b200 import binding
+    chunks = int((cfg1["edge_lanes"] * ((cfg1["edge_len_m"] + 127) // 128)).sum())
+    gran = binding.query_workspace(cfg1)
+    short = binding.query_workspace(dict(cfg1, params=dict(cfg1["params"], veh_len=3.5)))
+    tight = binding.query_workspace(dict(cfg1, params=dict(cfg1["params"], insert_clear_cells=3)))
+    monkeypatch.setenv("TS_CODE_GRANULE", "0")
+    forced = binding.query_workspace(cfg1)
+    assert short == tight == forced
+    saved = chunks * 128 - chunks * 32
+    assert 0 <= (short - gran) - saved < 512          # each plane is rounded up to 256 bytes
+
+
 def test_no_cpu_fallback(cfg1):
     """Without a CUDA device ts_create must fail loudly, not fall back."""
     import torch
